@@ -1,0 +1,146 @@
+/*
+ * ising.h -- C ABI of the B200-native exhaustive Ising enumerator
+ *            (hot path of arXiv 1904.03621, "Brute-forcing spin-glass problems with CUDA").
+ *
+ * What the library computes (PAPER.md:9 abstract, eq. (1), Algorithm 1):
+ * over all 2^N spin configurations of
+ *
+ *      H(s) = - sum_{i<j} J_ij s_i s_j - sum_i h_i s_i ,        s_i = +-1          (eq. 1)
+ *
+ * the S lowest (H, q) pairs, ascending under the total order (energy, state index).
+ * State encoding (eqs. (4),(5); PAPER.md:58 q = (s+1)/2):
+ * bit i of the 64-bit index q (bit 0 = least significant) is spin i; bit value 0 <-> s_i = -1,
+ * bit value 1 <-> s_i = +1. Spin i is row/column i of J and entry i of h (0-based).
+ *
+ * All work runs in hand-written sm_100a CUDA kernels enqueued on the caller's stream. There is
+ * no CPU fallback: without a CUDA device every compute entry point returns ISING_ERR_CUDA.
+ *
+ * Pointer arguments say in their name where they live: *_dev = device memory, *_host = host memory.
+ * The library never frees or retains caller buffers. Scratch is allocated per call with
+ * cudaMallocAsync on the caller's stream and released before returning.
+ * Every compute entry point SYNCHRONISES the stream before it returns (the launch loop is host
+ * sequenced), so outputs are valid on return. On any error the output buffers are left untouched
+ * (device variants) or unspecified (host variants) and a negative ISING_ERR_* code is returned.
+ * Nothing throws across this boundary. Calls on different streams may run concurrently.
+ */
+#ifndef ISING_H_
+#define ISING_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define ISING_OK               0
+#define ISING_ERR_NULL        -1   /* a required pointer is NULL */
+#define ISING_ERR_BAD_N       -2   /* N < 1 or N > ISING_N_MAX */
+#define ISING_ERR_BAD_S       -3   /* S < 1, S > number of states in the range, or S > ISING_S_MAX */
+#define ISING_ERR_NONFINITE   -4   /* NaN or Inf in J or h */
+#define ISING_ERR_ASYMMETRIC  -5   /* J[i*N+j] != J[j*N+i] */
+#define ISING_ERR_DIAGONAL    -6   /* J[i*N+i] != 0 (fields go in h, not on the diagonal) */
+#define ISING_ERR_BAD_RANGE   -7   /* q_begin >= q_end, q_end > 2^N, or bounds not multiples of 2^min(N,20) */
+#define ISING_ERR_CUDA        -8   /* a CUDA runtime call failed; see ising_last_error() */
+#define ISING_ERR_BAND        -9   /* guard band could not certify the result */
+#define ISING_ERR_INTERNAL   -10
+#define ISING_ERR_RANGE_W    -11   /* sum|J|+sum|h| is zero-scaled or too large/small to quantise */
+
+#define ISING_N_MAX   63
+#define ISING_S_MAX   65536
+
+/*
+ * ising_lowest -- the S lowest-energy states of the whole configuration space.
+ * (BASELINE.json north_star signature; Algorithm 1 is the paper's version of the same job.)
+ *
+ *   J_dev            [N*N] float64, row-major, symmetric, zero diagonal; edge {i,j} has coupling J[i*N+j]
+ *   h_dev            [N]   float64 fields
+ *   N                number of spins, 1 <= N <= ISING_N_MAX
+ *   S                number of states wanted, 1 <= S <= min(2^N, ISING_S_MAX)
+ *   states_out_dev   [S] uint64  state indices q, ascending by (energy, q)
+ *   energies_out_dev [S] float64 eq. (1) energies of those states, evaluated in fp64 in the fixed
+ *                    order "pairs i<j row-major, then fields" (integer-valued inputs give exact integers)
+ *   stream           a cudaStream_t passed as void* (NULL = default stream)
+ *
+ * Integer-valued (more generally: dyadic, exactly representable on the internal 2^-p grid) instances
+ * are enumerated exactly and the result is bit-exact. Other real-valued instances are enumerated on a
+ * fixed-point grid with a rigorous guard band and re-evaluated in fp64; if the
+ * band cannot certify completeness even after widening, ISING_ERR_BAND is returned.
+ */
+int ising_lowest(const double *J_dev, const double *h_dev, int N, int S,
+                 uint64_t *states_out_dev, double *energies_out_dev, void *stream);
+
+/*
+ * ising_lowest_range -- same, restricted to states q_begin <= q < q_end.
+ * Both bounds must be multiples of 2^min(N,20) (so for N <= 20 only the full range is legal).
+ * This is the unit of multi-GPU sharding, time slicing and checkpoint/resume (PAPER.md:85 chunks, eq. (6)).
+ */
+int ising_lowest_range(const double *J_dev, const double *h_dev, int N, int S,
+                       uint64_t q_begin, uint64_t q_end,
+                       uint64_t *states_out_dev, double *energies_out_dev, void *stream);
+
+/*
+ * ising_lowest_host -- end-to-end convenience: HOST buffers in, HOST buffers out. Copies J and h to
+ * the device, runs ising_lowest_range on `stream`, copies the S results back. Same semantics and codes.
+ */
+int ising_lowest_host(const double *J_host, const double *h_host, int N, int S,
+                      uint64_t q_begin, uint64_t q_end,
+                      uint64_t *states_out_host, double *energies_out_host, void *stream);
+
+/*
+ * ising_merge_lists -- the exchange step of range sharding ("low_en/low_st" merge).
+ * Input: n (state, energy) pairs (e.g. the concatenated per-range results); output: the S lowest under
+ * (energy, q), ascending. 1 <= S <= n. Duplicated states are NOT removed (ranges are disjoint).
+ */
+int ising_merge_lists(const uint64_t *states_in_dev, const double *energies_in_dev, int64_t n, int S,
+                      uint64_t *states_out_dev, double *energies_out_dev, void *stream);
+
+/*
+ * qubo_lowest -- QUBO entry point, eqs. (2),(3):
+ *      F(q) = - sum_{i<j} a_ij q_i q_j - sum_i b_i q_i ,   q_i in {0,1}
+ * a_dev [N*N] symmetric zero-diagonal, b_dev [N]. Converted on the device to the equivalent Ising
+ * instance (J = a/4, h_i = b_i/2 + sum_j a_ij/4, offset = -sum_i b_i/2 - sum_{i<j} a_ij/4) and
+ * enumerated by the same kernels; energies_out holds F(q) evaluated directly in fp64.
+ */
+int qubo_lowest(const double *a_dev, const double *b_dev, int N, int S,
+                uint64_t *states_out_dev, double *energies_out_dev, void *stream);
+
+/*
+ * ising_energies -- eq. (1) in fp64 for a list of n states (the re-evaluation kernel on its own).
+ */
+int ising_energies(const double *J_dev, const double *h_dev, int N,
+                   const uint64_t *states_dev, int64_t n, double *energies_out_dev, void *stream);
+
+/*
+ * Statistics of the last successful compute call made by the calling thread (for bench.py / tests).
+ * All counters refer to that one call.
+ */
+typedef struct ising_stats {
+    uint64_t configs;            /* configurations whose energy was computed (= q_end - q_begin per pass) */
+    uint64_t candidates;         /* (E, q) pairs that passed the threshold filter and reached a merge */
+    uint32_t kernel_launches;    /* kernels of this library launched */
+    uint32_t enum_launches;      /* of which enumeration kernels */
+    uint32_t passes;             /* 1, or more if the guard band had to be widened */
+    uint32_t split_retries;      /* launches re-run in halves after a candidate-buffer overflow */
+    int32_t  grid_exponent;      /* p: weights were quantised to multiples of 2^-p */
+    int32_t  exact;              /* 1 if the grid represents every weight exactly (integer / dyadic instance) */
+    double   epsilon;            /* rigorous bound on |grid energy - true energy| (0 if exact) */
+    double   enum_ms;            /* device time spent in enumeration kernels (CUDA events) */
+    double   total_ms;           /* device time of the whole call */
+    int32_t  keep;               /* K: candidates kept per list */
+    int32_t  inner_bits;         /* L: unrolled Gray bits per inner block */
+} ising_stats;
+
+int ising_get_last_stats(ising_stats *out_host);
+
+const char *ising_strerror(int status);
+const char *ising_last_error(void);   /* thread-local detail string of the last failure */
+int ising_version(void);
+
+/* FP32-FMA microbenchmark (the roofline denominator): runs a dependency-free FFMA kernel for roughly
+ * `ms_target` milliseconds on `stream` and writes the measured FMA/s (lane-FMAs per second, whole GPU). */
+int ising_fma_peak(double ms_target, double *fma_per_s_out_host, void *stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ISING_H_ */
