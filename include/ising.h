@@ -16,8 +16,9 @@
  * no CPU fallback: without a CUDA device every compute entry point returns ISING_ERR_CUDA.
  *
  * Pointer arguments say in their name where they live: *_dev = device memory, *_host = host memory.
- * The library never frees or retains caller buffers. Scratch is allocated per call with
- * cudaMallocAsync on the caller's stream and released before returning.
+ * The library never frees or retains caller buffers. Scratch (a 32 MiB candidate pool, the instance
+ * tables, a pinned control block) is allocated on first use per host thread and device, reused by that
+ * thread's later calls, and released by ising_release_workspace().
  * Every compute entry point SYNCHRONISES the stream before it returns (the launch loop is host
  * sequenced), so outputs are valid on return. On any error the output buffers are left untouched
  * (device variants) or unspecified (host variants) and a negative ISING_ERR_* code is returned.
@@ -139,6 +140,14 @@ int ising_version(void);
 /* FP32-FMA microbenchmark (the roofline denominator): runs a dependency-free FFMA kernel for roughly
  * `ms_target` milliseconds on `stream` and writes the measured FMA/s (lane-FMAs per second, whole GPU). */
 int ising_fma_peak(double ms_target, double *fma_per_s_out_host, void *stream);
+
+/* Same for the enumeration's inner operation, one fused integer add-min (SASS VIADDMNMX) per configuration:
+ * lane add-mins per second, whole GPU. This is the ALU ceiling the `roofline` of bench.py is quoted against
+ * (DESIGN.md "Roofline"). */
+int ising_addmin_peak(double ms_target, double *addmin_per_s_out_host, void *stream);
+
+/* Frees the calling thread's cached workspace (device pool, tables, pinned control block). Optional. */
+void ising_release_workspace(void);
 
 #ifdef __cplusplus
 }

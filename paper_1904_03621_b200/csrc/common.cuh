@@ -1,0 +1,119 @@
+// common.cuh -- shared declarations of the sm_100a CUDA path (product code; the CPU oracle shares nothing with it).
+//
+// Vocabulary:
+//   spin i <-> bit i of q (bit 0 = LSB); bit value 0 <-> s_i = -1, 1 <-> s_i = +1
+//   L  = "lo"   spins 0..LL-1          : per-thread register table V[2^LL]
+//   M  = "mid"  spins LL..LL+LM-1      : per-thread register table U[2^LM], shared table C[2^LM][2^LL]
+//   W  = "walk" spins LL+LM..+Lw-1     : walked by every thread in reflected Gray order
+//   T  = "thread" spins above          : lane, warp, block and launch-base bits; fixed per thread
+//   all energies in the kernels are int32 multiples of the grid 2^-p (stage.cu chooses p).
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace ising {
+
+constexpr int LL = 5;                    // lo bits
+constexpr int LM = 5;                    // mid bits
+constexpr int NLO = 1 << LL;
+constexpr int NMID = 1 << LM;
+constexpr int LOWBITS = LL + LM;         // bits enumerated by the add-min block
+constexpr int LW_MAX = 10;               // walk bits per thread (runtime Lw <= LW_MAX)
+constexpr int MIN_CHUNK_BITS = LOWBITS + 5;   // one warp, no walk: 2^15 configurations
+constexpr int N_DIRECT_MAX = MIN_CHUNK_BITS - 1;   // N <= 14: direct kernel
+constexpr int WQ_BITS = 27;              // sum|Jq| + sum|hq| <= 2^27 grid units
+constexpr int TAU_INF = 0x3fffffff;      // "no threshold yet"; every grid energy is far below it
+constexpr unsigned long long Q_MAX = ~0ull;
+
+constexpr unsigned POOL_CAP_LOG2 = 21;
+constexpr unsigned POOL_CAP = 1u << POOL_CAP_LOG2;     // entries in the candidate pool
+constexpr unsigned KEEP_CAP = 1u << 20;                // most entries kept after a selection
+constexpr int SORT_TILE = 4096;                        // entries sorted by one block in shared memory
+constexpr int SORT_THREADS = 1024;
+
+// One candidate: sortable 64-bit key (grid energy or fp64 energy, order preserving) and the state index.
+struct __align__(16) Entry {
+    unsigned long long key;
+    unsigned long long q;
+};
+
+__host__ __device__ inline bool entry_less(const Entry& a, const Entry& b)
+{
+    return a.key < b.key || (a.key == b.key && a.q < b.q);
+}
+__host__ __device__ inline unsigned long long key_from_i32(int e)
+{
+    return (unsigned long long)((unsigned)e ^ 0x80000000u);
+}
+__host__ __device__ inline int i32_from_key(unsigned long long k)
+{
+    return (int)((unsigned)k ^ 0x80000000u);
+}
+__device__ inline unsigned long long key_from_f64(double x)
+{
+    x += 0.0;                                    // -0.0 -> +0.0
+    unsigned long long b = (unsigned long long)__double_as_longlong(x);
+    return (b >> 63) ? ~b : (b | 0x8000000000000000ull);
+}
+__device__ inline double f64_from_key(unsigned long long k)
+{
+    unsigned long long b = (k >> 63) ? (k & 0x7fffffffffffffffull) : ~k;
+    return __longlong_as_double((long long)b);
+}
+
+// Device-resident control block of one call; the host reads it back through pinned memory.
+struct Ctrl {
+    int status;            // ISING_OK or an ISING_ERR_* found by the staging kernel
+    int p;                 // grid exponent: weights are multiples of 2^-p
+    int exact;             // 1: every weight is on the grid (epsilon = 0)
+    int band;              // guard band in grid units: candidates are kept up to E_S + band
+    double epsilon;        // bound on |grid energy * 2^-p - eq.(1) energy|
+    double W;              // sum_{i<j}|J_ij| + sum_i|h_i|
+    unsigned count;        // entries in the pool (kept prefix + new candidates); may exceed POOL_CAP = overflow
+    unsigned kept;         // entries of the sorted prefix after the last selection
+    int tauE;              // filter threshold (grid units)
+    int pad0;
+    unsigned long long tauQ;   // ties on tauE pass only for q < tauQ
+    unsigned band_overflow;    // selection wanted to keep more than KEEP_CAP entries
+    unsigned pad1;
+    unsigned long long candidates;   // running total of pushes
+};
+
+// Instance tables in grid units, built once per call by build_tables (stage.cu).
+struct Tables {
+    int Jq[64 * 64];               // quantised couplings, row-major, N x N used with stride 64
+    int hq[64];
+    int C[NMID * NLO];             // C[mid][lo]  = -4 sum_{i in lo, j in mid} Jq_ij        (eq. (2) pair terms)
+    int QL[NLO];                   // QL[lo]      = -4 sum_{i<j in lo} Jq_ij
+    int QM[NMID];                  // QM[mid]     = -4 sum_{i<j in mid} Jq_ij
+    int DV[LW_MAX * 2 * NLO];      // DV[k][sb][lo]  = sgn * -4 sum_{i in lo} Jq[i][w_k],  sgn = sb ? +1 : -1
+    int DU[LW_MAX * 2 * NMID];     // DU[k][sb][mid] = sgn * -4 sum_{j in mid} Jq[j][w_k]
+    int DW[1 << LW_MAX];           // DW[t] = -sgn_t * 4 sum_{j in R_t} Jq[w_k][w_j]   (walk-internal part of step t)
+};
+
+struct Geometry {
+    int N;
+    int Lw;                        // walk bits of this launch
+    unsigned long long base;       // first state of the launch (aligned to the launch size)
+};
+
+// stage.cu
+void launch_stage(const double* J, const double* h, int N, Tables* tab, Ctrl* ctrl, cudaStream_t st,
+                  double extra_eps_rel);
+void launch_qubo_to_ising(const double* a, const double* b, int N, double* J, double* h, cudaStream_t st);
+// enumerate.cu
+void launch_enumerate(const Tables* tab, Ctrl* ctrl, Entry* pool, int N, int Lw,
+                      unsigned long long base, unsigned nthreads, cudaStream_t st);
+void launch_direct(const Tables* tab, Ctrl* ctrl, Entry* pool, int N, cudaStream_t st);
+// select.cu
+int  launch_select(Entry* pool, Ctrl* ctrl, unsigned n, int S, cudaStream_t st);     // returns kernels launched
+int  launch_final(const double* J, const double* h, int N, int mode, Entry* pool, unsigned m, int S,
+                  unsigned long long* states_out, double* energies_out, cudaStream_t st);
+void launch_energies(const double* J, const double* h, int N, int mode, const unsigned long long* states,
+                     long long n, double* out, cudaStream_t st);
+int  launch_merge_lists(const unsigned long long* states, const double* energies, long long n, int S, Entry* scratch,
+                        unsigned long long* states_out, double* energies_out, cudaStream_t st);
+// peak.cu
+double run_fma_peak(double ms_target, cudaStream_t st, int which);
+
+}  // namespace ising

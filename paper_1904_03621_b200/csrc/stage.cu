@@ -1,0 +1,205 @@
+// stage.cu -- SURVEY.md section 8 row a1: validate the instance, put it on a power-of-two grid, build the tables.
+//
+// The enumeration works in exact integer arithmetic on the quantised instance (Jq, hq) = rint((J, h) * 2^p):
+// every sum the kernels form is an int32 multiple of 2^-p, so there is no accumulation error and the only
+// difference to eq. (1) is the input rounding, bounded rigorously by
+//      epsilon = sum_{i<j} |Jq_ij 2^-p - J_ij| + sum_i |hq_i 2^-p - h_i|.
+// Integer / dyadic instances have epsilon = 0 and are enumerated exactly.
+//
+// Tables are the paper's QUBO form, eqs. (2),(3), taken relative to a base state q0 whose
+// L, M and W bits are 0:   E(q0 + A) = E(q0) - 2 sum_{i in A} Phi_i(q0) - 4 sum_{i<j in A} J_ij
+// with Phi_i(q0) = h_i + sum_j J_ij s_j(q0) the local field at the base state (a_ij = 4 J_ij of eq. (3)).
+#include "common.cuh"
+#include "../../include/ising.h"
+
+namespace ising {
+
+__global__ void __launch_bounds__(256) stage_kernel(const double* __restrict__ J, const double* __restrict__ h, int N,
+                                                    Tables* __restrict__ tab, Ctrl* __restrict__ ctrl,
+                                                    double extra_eps_rel)
+{
+    __shared__ int s_status;
+    __shared__ int s_p;
+    __shared__ double s_red[256];
+    const int tid = threadIdx.x;
+    constexpr int NO_ERROR_YET = -1000;
+    if (tid == 0) s_status = NO_ERROR_YET;
+    __syncthreads();
+
+    // ---- validation: finite, symmetric, zero diagonal (include/ising.h error codes; most severe wins) ----
+    int bad = ISING_OK;
+    for (int idx = tid; idx < N * N; idx += blockDim.x) {
+        int i = idx / N, j = idx % N;
+        double v = J[idx];
+        if (!isfinite(v)) bad = ISING_ERR_NONFINITE;
+        else if (i == j) { if (v != 0.0 && bad != ISING_ERR_NONFINITE) bad = ISING_ERR_DIAGONAL; }
+        else if (!(v == J[j * N + i]) && bad == ISING_OK) bad = ISING_ERR_ASYMMETRIC;
+    }
+    for (int i = tid; i < N; i += blockDim.x)
+        if (!isfinite(h[i])) bad = ISING_ERR_NONFINITE;
+    // codes are negative; NONFINITE (-4) outranks ASYMMETRIC (-5) outranks DIAGONAL (-6): report the max
+    if (bad != ISING_OK) atomicMax(&s_status, bad);
+    __syncthreads();
+    if (s_status != NO_ERROR_YET) {
+        if (tid == 0) ctrl->status = s_status;
+        return;
+    }
+
+    // ---- W = sum_{i<j}|J_ij| + sum_i|h_i| : per-thread partials, then a fixed-order tree (deterministic) ----
+    double part = 0.0;
+    for (int idx = tid; idx < N * N; idx += blockDim.x) {
+        int i = idx / N, j = idx % N;
+        if (i < j) part += fabs(J[idx]);
+    }
+    for (int i = tid; i < N; i += blockDim.x) part += fabs(h[i]);
+    s_red[tid] = part;
+    __syncthreads();
+    for (int s = 128; s > 0; s >>= 1) {
+        if (tid < s) s_red[tid] += s_red[tid + s];
+        __syncthreads();
+    }
+    const double W = s_red[0];
+    if (tid == 0) {
+        int p = 0, st = ISING_OK;
+        if (!isfinite(W)) st = ISING_ERR_RANGE_W;
+        else if (W > 0.0) {
+            int e;
+            frexp(W * (1.0 + 1e-9), &e);          // W < 2^e  (the factor covers the rounding of the fp64 sum)
+            p = WQ_BITS - e;                      // sum of |rint(x 2^p)| <= W 2^p + (#terms)/2 < 2^27 + 2^11
+            if (p > 1000 || p < -1000) st = ISING_ERR_RANGE_W;
+        }
+        s_p = p;
+        s_status = st;
+    }
+    __syncthreads();
+    if (s_status != ISING_OK) { if (tid == 0) ctrl->status = s_status; return; }
+    const int p = s_p;
+
+    // ---- quantise; accumulate the rounding error of each weight that enters eq. (1) once ----
+    double err = 0.0;
+    for (int idx = tid; idx < 64 * 64; idx += blockDim.x) {
+        int i = idx >> 6, j = idx & 63;
+        int q = 0;
+        if (i < N && j < N && i != j) {
+            double v = J[i * N + j];
+            double r = rint(ldexp(v, p));
+            q = (int)r;
+            if (i < j) err += fabs(ldexp(r, -p) - v);
+        }
+        tab->Jq[idx] = q;
+    }
+    for (int i = tid; i < 64; i += blockDim.x) {
+        int q = 0;
+        if (i < N) {
+            double v = h[i];
+            double r = rint(ldexp(v, p));
+            q = (int)r;
+            err += fabs(ldexp(r, -p) - v);
+        }
+        tab->hq[i] = q;
+    }
+    s_red[tid] = err;
+    __syncthreads();
+    for (int s = 128; s > 0; s >>= 1) {
+        if (tid < s) s_red[tid] += s_red[tid + s];
+        __syncthreads();
+    }
+    if (tid == 0) {
+        double eps = s_red[0] + extra_eps_rel * W;     // extra: rounding done before staging (qubo_lowest)
+        int exact = (eps == 0.0);
+        int band = 0;
+        if (!exact) {
+            eps *= (1.0 + 1e-9);                               // rounding of the error sum itself
+            double b = ceil(ldexp(2.0 * eps, p)) + 1.0;        // 2 epsilon in grid units, rounded up
+            band = (b < 1.0e9) ? (int)b : 1000000000;
+        }
+        ctrl->status = ISING_OK;
+        ctrl->p = p;
+        ctrl->exact = exact;
+        ctrl->band = band;
+        ctrl->epsilon = eps;
+        ctrl->W = W;
+        ctrl->count = 0;
+        ctrl->kept = 0;
+        ctrl->tauE = TAU_INF;
+        ctrl->tauQ = Q_MAX;
+        ctrl->band_overflow = 0;
+        ctrl->candidates = 0;
+    }
+}
+
+// Tables of the QUBO form relative to the base state (see file header). One block; thread-per-entry loops.
+__global__ void __launch_bounds__(256) tables_kernel(Tables* __restrict__ tab, const Ctrl* __restrict__ ctrl, int N)
+{
+    if (ctrl->status != ISING_OK) return;
+    const int tid = threadIdx.x;
+    const int* Jq = tab->Jq;
+    auto Jat = [&](int i, int j) -> int { return (i < N && j < N) ? Jq[i * 64 + j] : 0; };
+
+    for (int idx = tid; idx < NMID * NLO; idx += blockDim.x) {
+        int mid = idx / NLO, lo = idx % NLO, acc = 0;
+        for (int i = 0; i < LL; ++i) if (lo >> i & 1)
+            for (int j = 0; j < LM; ++j) if (mid >> j & 1) acc += Jat(i, LL + j);
+        tab->C[idx] = -4 * acc;
+    }
+    for (int lo = tid; lo < NLO; lo += blockDim.x) {
+        int acc = 0;
+        for (int i = 0; i < LL; ++i) if (lo >> i & 1)
+            for (int j = i + 1; j < LL; ++j) if (lo >> j & 1) acc += Jat(i, j);
+        tab->QL[lo] = -4 * acc;
+    }
+    for (int mid = tid; mid < NMID; mid += blockDim.x) {
+        int acc = 0;
+        for (int i = 0; i < LM; ++i) if (mid >> i & 1)
+            for (int j = i + 1; j < LM; ++j) if (mid >> j & 1) acc += Jat(LL + i, LL + j);
+        tab->QM[mid] = -4 * acc;
+    }
+    for (int idx = tid; idx < LW_MAX * 2 * NLO; idx += blockDim.x) {
+        int k = idx / (2 * NLO), sb = (idx / NLO) & 1, lo = idx % NLO, acc = 0;
+        for (int i = 0; i < LL; ++i) if (lo >> i & 1) acc += Jat(i, LOWBITS + k);
+        tab->DV[idx] = (sb ? -4 : 4) * acc;
+    }
+    for (int idx = tid; idx < LW_MAX * 2 * NMID; idx += blockDim.x) {
+        int k = idx / (2 * NMID), sb = (idx / NMID) & 1, mid = idx % NMID, acc = 0;
+        for (int j = 0; j < LM; ++j) if (mid >> j & 1) acc += Jat(LL + j, LOWBITS + k);
+        tab->DU[idx] = (sb ? -4 : 4) * acc;
+    }
+    for (int t = tid; t < (1 << LW_MAX); t += blockDim.x) {
+        int v = 0;
+        if (t > 0) {
+            int k = __ffs(t) - 1;
+            int gnew = t ^ (t >> 1);
+            int sgn = (gnew >> k & 1) ? 1 : -1;
+            int R = gnew & ~(1 << k);
+            int acc = 0;
+            for (int j = 0; j < LW_MAX; ++j) if (R >> j & 1) acc += Jat(LOWBITS + k, LOWBITS + j);
+            v = -sgn * 4 * acc;
+        }
+        tab->DW[t] = v;
+    }
+}
+
+void launch_stage(const double* J, const double* h, int N, Tables* tab, Ctrl* ctrl, cudaStream_t st,
+                  double extra_eps_rel)
+{
+    stage_kernel<<<1, 256, 0, st>>>(J, h, N, tab, ctrl, extra_eps_rel);
+    tables_kernel<<<1, 256, 0, st>>>(tab, ctrl, N);
+}
+
+// QUBO -> Ising, eqs. (2),(3) inverted: J = a/4, h_i = b_i/2 + sum_j a_ij/4.
+__global__ void qubo_to_ising_kernel(const double* __restrict__ a, const double* __restrict__ b, int N,
+                                     double* __restrict__ J, double* __restrict__ h)
+{
+    for (int idx = threadIdx.x; idx < N * N; idx += blockDim.x) J[idx] = 0.25 * a[idx];
+    for (int i = threadIdx.x; i < N; i += blockDim.x) {
+        double acc = 0.0;
+        for (int j = 0; j < N; ++j) if (j != i) acc += a[i * N + j];
+        h[i] = 0.5 * b[i] + 0.25 * acc;
+    }
+}
+void launch_qubo_to_ising(const double* a, const double* b, int N, double* J, double* h, cudaStream_t st)
+{
+    qubo_to_ising_kernel<<<1, 256, 0, st>>>(a, b, N, J, h);
+}
+
+}  // namespace ising
