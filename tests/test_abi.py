@@ -1,0 +1,104 @@
+"""Host-side checks of the C-ABI library: it builds for sm_100a, loads, exports every symbol include/ising.h
+declares, and its argument validation (which runs before any CUDA call) returns the documented codes.
+No compute call succeeds here without a GPU -- and the test asserts that it fails loudly, not silently."""
+import ctypes
+import os
+import re
+import shutil
+
+import numpy as np
+import pytest
+
+from conftest import ROOT, has_cuda
+
+nvcc_missing = shutil.which("nvcc") is None and not os.path.exists("/usr/local/cuda/bin/nvcc")
+pytestmark = pytest.mark.skipif(nvcc_missing, reason="nvcc not available")
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_1904_03621_b200 import build, binding
+    build.build()
+    return binding.load()
+
+
+def _declared_functions():
+    text = open(os.path.join(ROOT, "include", "ising.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    names = re.findall(r"\b(?:int|void|const char \*)\s*\*?\s*((?:ising|qubo)_\w+)\s*\(", text)
+    return sorted(set(names))
+
+
+def test_header_symbols_exported(lib):
+    from paper_1904_03621_b200 import binding
+    declared = _declared_functions()
+    assert len(declared) >= 13
+    assert sorted(binding.EXPORTS) == declared
+    for name in declared:
+        assert hasattr(lib, name), f"{name} declared in include/ising.h but not exported"
+
+
+def test_version_and_strerror(lib):
+    from paper_1904_03621_b200 import binding
+    assert binding.version() >= 100
+    assert binding.strerror(0) == "ok"
+    for code in range(-11, 0):
+        assert binding.strerror(code) not in ("ok", "unknown status")
+    assert binding.strerror(-99) == "unknown status"
+
+
+def test_argument_validation_precedes_cuda(lib):
+    """NULL / N / range / S errors are decided on the host before the first CUDA call."""
+    from paper_1904_03621_b200 import binding as B
+    J = np.zeros((20, 20)); h = np.zeros(20)
+    q = np.zeros(16, dtype=np.uint64); e = np.zeros(16)
+    Jp, hp, qp, ep = J.ctypes.data, h.ctypes.data, q.ctypes.data, e.ctypes.data
+    f = lib.ising_lowest_host
+    assert f(None, hp, 20, 16, 0, 1 << 20, qp, ep, None) == B.ERR_NULL
+    assert f(Jp, hp, 20, 16, 0, 1 << 20, None, ep, None) == B.ERR_NULL
+    assert f(Jp, hp, 0, 16, 0, 1, qp, ep, None) == B.ERR_BAD_N
+    assert f(Jp, hp, 64, 16, 0, 1 << 20, qp, ep, None) == B.ERR_BAD_N
+    assert f(Jp, hp, 20, 16, 0, 1 << 19, qp, ep, None) == B.ERR_BAD_RANGE      # N <= 20: only the full range
+    assert f(Jp, hp, 20, 16, 0, (1 << 20) + 1, qp, ep, None) == B.ERR_BAD_RANGE
+    assert f(Jp, hp, 20, 0, 0, 1 << 20, qp, ep, None) == B.ERR_BAD_S
+    assert f(Jp, hp, 20, B.S_MAX + 1, 0, 1 << 20, qp, ep, None) == B.ERR_BAD_S
+    assert lib.ising_lowest(Jp, hp, 99, 16, qp, ep, None) == B.ERR_BAD_N
+    assert lib.ising_merge_lists(None, ep, 4, 2, qp, ep, None) == B.ERR_NULL
+    assert lib.ising_merge_lists(qp, ep, 4, 5, qp, ep, None) == B.ERR_BAD_S
+    assert lib.ising_energies(Jp, hp, 20, None, 4, ep, None) == B.ERR_NULL
+    assert lib.ising_get_last_stats(None) == B.ERR_NULL
+    assert lib.ising_fma_peak(1.0, None, None) == B.ERR_NULL
+    # N = 24: ranges must be multiples of 2^20
+    J = np.zeros((24, 24)); h = np.zeros(24)
+    assert f(J.ctypes.data, h.ctypes.data, 24, 16, 1 << 19, 1 << 21, qp, ep, None) == B.ERR_BAD_RANGE
+    assert f(J.ctypes.data, h.ctypes.data, 24, 16, 1 << 21, 1 << 20, qp, ep, None) == B.ERR_BAD_RANGE
+    assert b"range" in lib.ising_last_error()
+
+
+@pytest.mark.skipif(has_cuda(), reason="only meaningful on a box without a GPU")
+def test_no_cpu_fallback_without_gpu(lib):
+    """Without a CUDA device a compute call must fail with ISING_ERR_CUDA, never produce a result on the host."""
+    from paper_1904_03621_b200 import binding as B
+    J = np.zeros((8, 8)); h = np.ones(8)
+    q = np.full(4, 12345, dtype=np.uint64); e = np.full(4, 7.0)
+    rc = lib.ising_lowest_host(J.ctypes.data, h.ctypes.data, 8, 4, 0, 256, q.ctypes.data, e.ctypes.data, None)
+    assert rc == B.ERR_CUDA
+    assert q.tolist() == [12345] * 4 and e.tolist() == [7.0] * 4      # outputs untouched
+    with pytest.raises(B.IsingError):
+        B._check(rc, "ising_lowest_host")
+
+
+def test_product_does_not_import_oracle():
+    """The product path shares nothing with oracle/: no import, include or load, in either direction."""
+    pkg = os.path.join(ROOT, "paper_1904_03621_b200")
+    bad_in_product = re.compile(r"^\s*(from|import)\s+oracle\b|#include\s*[\"<][^\n]*oracle|liboracle", re.M)
+    for dirpath, _, files in os.walk(pkg):
+        for fn in files:
+            if fn.endswith((".py", ".cu", ".cuh", ".h", ".cpp")):
+                text = open(os.path.join(dirpath, fn)).read()
+                assert not bad_in_product.search(text), fn
+    bad_in_oracle = re.compile(r"^\s*(from|import)\s+paper_1904_03621_b200|#include\s*\"\.\./|libising", re.M)
+    for fn in os.listdir(os.path.join(ROOT, "oracle")):
+        if fn.endswith((".py", ".c", ".h")):
+            text = open(os.path.join(ROOT, "oracle", fn)).read()
+            assert not bad_in_oracle.search(text), fn

@@ -1,0 +1,314 @@
+"""Parity of the CUDA path (through the C ABI) with the CPU oracle, element by element, on seeded inputs.
+All tests here need a B200: run with  python -m pytest tests -m gpu."""
+import os
+
+import numpy as np
+import pytest
+
+from checker import assert_exact, assert_real, load_golden
+from oracle import oracle
+from paper_1904_03621_b200 import instances as I
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_1904_03621_b200 import binding, build
+    build.build()
+    binding.load()
+    return binding
+
+
+def gpu_lowest(B, J, h, S, q_begin=None, q_end=None):
+    if q_begin is None:
+        q, e = B.ising_lowest(J, h, S)
+    else:
+        q, e = B.ising_lowest_range(J, h, S, q_begin, q_end)
+    return B.states_to_numpy(q), e.cpu().numpy()
+
+
+# ---------- the paper's Listing 1 (tests/golden/listing1.txt, by hand) ----------
+def test_listing1(B, golden_dir):
+    rows = [l.split() for l in open(os.path.join(golden_dir, "listing1.txt")) if l.strip() and l[0] != "#"]
+    J = np.zeros((2, 2)); J[0, 1] = J[1, 0] = -0.2
+    h = np.array([-1.0, 0.0])
+    q, e = gpu_lowest(B, J, h, 4)
+    assert q.tolist() == [int(r[0]) for r in rows]
+    np.testing.assert_allclose(e, [float(r[1]) for r in rows], rtol=0, atol=1e-15)
+
+
+# ---------- small sizes, every code path: direct kernel (N <= 14), single-warp launches, ragged plans ----------
+@pytest.mark.parametrize("N", [1, 2, 3, 5, 9, 13, 14, 15, 16, 17, 19, 20, 21, 23])
+def test_small_real_vs_oracle(B, N):
+    J, h = I.complete_gaussian(N, seed=100 + N)
+    for S in sorted({1, min(7, 1 << N), min(100, 1 << N), min(1 << N, 4096)}):
+        q, e = gpu_lowest(B, J, h, S)
+        qo, eo = oracle.lowest(J, h, S)
+        assert_exact(q, e, qo, eo)          # same fp64 summation order on both sides: bit-exact
+
+
+@pytest.mark.parametrize("N,wmax,density", [(4, 1, 1.0), (10, 1, 0.3), (14, 2, 0.5), (15, 1, 0.2), (18, 3, 0.5),
+                                            (20, 1, 0.15), (22, 2, 1.0), (24, 1, 0.1)])
+def test_small_integer_heavy_ties(B, N, wmax, density):
+    J, h = I.random_integer(N, seed=7 * N, wmax=wmax, density=density)
+    for S in (1, min(64, 1 << N), min(1000, 1 << N)):
+        q, e = gpu_lowest(B, J, h, S)
+        qo, eo = oracle.lowest(J, h, S)
+        assert_exact(q, e, qo, eo)
+        assert B.last_stats().exact
+
+
+def test_full_sort_S_equals_all_states(B):
+    for N, integer in ((12, True), (14, False), (16, True), (16, False)):
+        J, h = I.random_integer(N, seed=N, wmax=2) if integer else I.complete_gaussian(N, seed=N)
+        S = 1 << N
+        q, e = gpu_lowest(B, J, h, S)
+        qo, eo = oracle.lowest(J, h, S)
+        assert_exact(q, e, qo, eo)
+
+
+def test_large_S(B):
+    J, h = I.complete_gaussian(18, seed=181)
+    S = 50000
+    q, e = gpu_lowest(B, J, h, S)
+    qo, eo = oracle.lowest(J, h, S)
+    assert_exact(q, e, qo, eo)
+    J, h = I.random_integer(19, seed=191, wmax=1, density=0.3)
+    q, e = gpu_lowest(B, J, h, B.S_MAX)
+    qo, eo = oracle.lowest(J, h, B.S_MAX)
+    assert_exact(q, e, qo, eo)
+
+
+def test_degenerate_instances(B):
+    # all-zero instance: every energy 0, order purely by q
+    for N in (6, 16, 22):
+        q, e = gpu_lowest(B, np.zeros((N, N)), np.zeros(N), min(50, 1 << N))
+        assert q.tolist() == list(range(min(50, 1 << N))) and not e.any()
+    # non-dyadic weights with massive exact ties (guard-band mode keeps whole levels)
+    N = 20
+    h = np.full(N, 0.1); J = np.zeros((N, N))
+    q, e = gpu_lowest(B, J, h, 300)
+    qo, eo = oracle.lowest(J, h, 300)
+    assert_exact(q, e, qo, eo)
+    assert not B.last_stats().exact
+    # energies strictly decreasing in q: every launch beats everything before it -> pool overflow and split path
+    N = 24
+    h = 2.0 ** np.arange(N); J = np.zeros((N, N))
+    q, e = gpu_lowest(B, J, h, 1000)
+    assert q.tolist() == list(range((1 << N) - 1, (1 << N) - 1001, -1))
+    assert B.last_stats().split_retries > 0
+
+
+# ---------- closed forms ----------
+@pytest.mark.parametrize("N", [16, 25, 33])
+def test_ferromagnet_and_mattis(B, N):
+    full = (1 << N) - 1
+    E0 = -N * (N - 1) / 2
+    E1 = -((N - 2) ** 2 - N) / 2
+    J, h, xi = I.mattis(N, seed=N)
+    q_xi = sum(1 << i for i in range(N) if xi[i] > 0)
+    exp = [(E0, q_xi), (E0, full ^ q_xi)]
+    exp += [(E1, q_xi ^ (1 << i)) for i in range(N)] + [(E1, full ^ q_xi ^ (1 << i)) for i in range(N)]
+    exp = sorted(exp)
+    q, e = gpu_lowest(B, J, h, len(exp))
+    assert [(float(ee), int(qq)) for qq, ee in zip(q, e)] == exp
+    J, h = I.ferromagnet(N)
+    q, e = gpu_lowest(B, J, h, 2)
+    assert q.tolist() == [0, full] and e.tolist() == [E0, E0]
+
+
+def test_fields_only_sign_convention(B):
+    """G2: eq. (1) as printed: the ground state of a fields-only instance has s_i = +sign(h_i)."""
+    N = 30
+    J, h = I.fields_only(N, seed=5)
+    q, e = gpu_lowest(B, J, h, 2)
+    q0 = sum(1 << i for i in range(N) if h[i] > 0)
+    w = int(np.argmin(np.abs(h)))
+    assert q.tolist() == [q0, q0 ^ (1 << w)]
+    assert abs(e[0] + np.abs(h).sum()) < 1e-12 and abs(e[1] - e[0] - 2 * abs(h[w])) < 1e-12
+
+
+# ---------- BASELINE.json configs against stored oracle outputs ----------
+def test_config1_golden(B, golden_dir):
+    c = I.baseline_config(1)
+    qo, eo = load_golden(os.path.join(golden_dir, "cfg1.txt"))
+    q, e = gpu_lowest(B, c.J, c.h, c.S)
+    assert_exact(q, e, qo[:c.S], eo[:c.S])
+    assert_real(q, e, qo, eo, np.abs(np.triu(c.J, 1)).sum() + np.abs(c.h).sum(), c.S)
+
+
+@pytest.mark.parametrize("k", [2, 3])
+def test_config_golden(B, golden_dir, k):
+    path = os.path.join(golden_dir, f"cfg{k}.txt")
+    if not os.path.exists(path):
+        pytest.skip(f"{path} not generated yet (tests/golden/make_goldens.py {k})")
+    c = I.baseline_config(k)
+    qo, eo = load_golden(path)
+    assert c.sha256() in open(path).read()
+    q, e = gpu_lowest(B, c.J, c.h, c.S)
+    assert_exact(q, e, qo[:c.S], eo[:c.S])
+
+
+# ---------- sub-range parity at the full sizes (48-bit index assembly, chunk seams) ----------
+@pytest.mark.parametrize("k,unit_log2,units", [(3, 20, 6), (4, 20, 5), (5, 20, 3), (5, 21, 2)])
+def test_subrange_parity(B, k, unit_log2, units):
+    c = I.baseline_config(k)
+    rng = np.random.default_rng(1000 + k)
+    top = (1 << c.N) >> unit_log2
+    for _ in range(2):
+        lo = int(rng.integers(0, top - units)) << unit_log2
+        hi = lo + (units << unit_log2)
+        S = min(c.S, 200)
+        q, e = gpu_lowest(B, c.J, c.h, S, lo, hi)
+        qo, eo = oracle.lowest(c.J, c.h, S, lo, hi)
+        assert_exact(q, e, qo, eo)
+
+
+def test_range_split_and_merge(B):
+    import torch
+    c = I.baseline_config(3)
+    S = c.S
+    q_full, e_full = B.ising_lowest(c.J, c.h, S)
+    parts = []
+    edges = [0, 1 << 33, (1 << 33) + (1 << 20), 3 << 34, 1 << 36]
+    for lo, hi in zip(edges[:-1], edges[1:]):
+        parts.append(B.ising_lowest_range(c.J, c.h, min(S, hi - lo), lo, hi))
+    qs = torch.cat([p[0] for p in parts]); es = torch.cat([p[1] for p in parts])
+    q_m, e_m = B.ising_merge_lists(qs, es, S)
+    assert torch.equal(q_m, q_full) and torch.equal(e_m, e_full)
+
+
+# ---------- necessary conditions and metamorphic relations where no oracle run is possible ----------
+def _neighbour_check(J, h, q, e, nflip=2, seeds=None):
+    """Every 1- and 2-flip neighbour of a returned state that is below the S-th entry must be in the list."""
+    N = len(h)
+    have = set(int(x) for x in q)
+    last = (float(e[-1]), int(q[-1]))
+    cand = set()
+    for x in (have if seeds is None else [int(x) for x in q[:seeds]]):
+        for i in range(N):
+            cand.add(x ^ (1 << i))
+            if nflip >= 2:
+                for j in range(i + 1, N):
+                    cand.add(x ^ (1 << i) ^ (1 << j))
+    cand = np.array(sorted(cand - have), dtype=np.uint64)
+    en = oracle.energies_of(J, h, cand)
+    for x, ee in zip(cand, en):
+        assert (float(ee), int(x)) > last, f"missed neighbour {int(x)} with energy {ee}"
+
+
+def test_config4_full_run_properties(B):
+    c = I.baseline_config(4)
+    q, e = gpu_lowest(B, c.J, c.h, c.S)
+    st = B.last_stats()
+    assert st.exact and st.configs == 1 << c.N
+    np.testing.assert_array_equal(oracle.energies_of(c.J, c.h, q), e)       # energies are the oracle's, state by state
+    pairs = list(zip(e.tolist(), q.tolist()))
+    assert pairs == sorted(pairs) and len(set(q.tolist())) == c.S
+    assert all(float(x).is_integer() for x in e)
+    _neighbour_check(c.J, c.h, q, e, nflip=2, seeds=100)
+    # metamorphic: gauge transformation  J'_ij = g_i g_j J_ij, h'_i = g_i h_i  <=>  q' = q xor mask, same energies
+    rng = np.random.default_rng(4)
+    g = 2.0 * rng.integers(0, 2, size=c.N) - 1.0
+    mask = sum(1 << i for i in range(c.N) if g[i] < 0)
+    q2, e2 = gpu_lowest(B, c.J * np.outer(g, g), c.h * g, c.S)
+    # ties on the last level are cut by q order, which the gauge changes: compare what is unique (levels below it)
+    assert e2.tolist() == e.tolist()
+    inner = [p for p in pairs if p[0] < e[-1]]
+    assert sorted(p for p in zip(e2.tolist(), (q2 ^ np.uint64(mask)).tolist()) if p[0] < e[-1]) == inner
+    np.testing.assert_array_equal(oracle.energies_of(c.J, c.h, q2 ^ np.uint64(mask)), e2)
+
+
+def test_config3_metamorphic(B):
+    c = I.baseline_config(3)
+    q, e = gpu_lowest(B, c.J, c.h, c.S)
+    np.testing.assert_array_equal(oracle.energies_of(c.J, c.h, q), e)
+    _neighbour_check(c.J, c.h, q, e, nflip=2)
+    full = np.uint64((1 << c.N) - 1)
+    # (J, -h): q' = ~q, energies identical
+    q2, e2 = gpu_lowest(B, c.J, -c.h, c.S)
+    assert (q2 ^ full).tolist() == q.tolist() and e2.tolist() == e.tolist()
+    # scaling by 2^m is exact
+    q3, e3 = gpu_lowest(B, c.J * 8.0, c.h * 8.0, c.S)
+    assert q3.tolist() == q.tolist() and e3.tolist() == (e * 8.0).tolist()
+    # spin relabelling: moves spins between the lo / mid / walk / thread roles
+    rng = np.random.default_rng(3)
+    perm = rng.permutation(c.N)                     # new spin a is old spin perm[a]
+    Jp = c.J[np.ix_(perm, perm)]; hp = c.h[perm]
+    q4, e4 = gpu_lowest(B, Jp, hp, c.S)
+    back = np.zeros(c.S, dtype=np.uint64)
+    for a in range(c.N):
+        back |= ((q4 >> np.uint64(a)) & np.uint64(1)) << np.uint64(perm[a])
+    assert back.tolist() == q.tolist()
+    np.testing.assert_allclose(e4, e, rtol=1e-12, atol=0)
+
+
+def test_two_blocks_pair_sums_36(B):
+    """P8 at a size the oracle reaches: block-diagonal J, spectrum = pair sums of the two blocks' spectra."""
+    NA = NB = 18
+    J, h = I.two_blocks(NA, NB, seed=321)
+    eA = oracle.energies_range(J[:NA, :NA], h[:NA], 0, 1 << NA)
+    eB = oracle.energies_range(J[NA:, NA:], h[NA:], 0, 1 << NB)
+    ia = np.argsort(eA, kind="stable")[:300]; ib = np.argsort(eB, kind="stable")[:300]
+    tot = eA[ia][None, :] + eB[ib][:, None]
+    qq = ia[None, :].astype(np.uint64) | (ib[:, None].astype(np.uint64) << np.uint64(NA))
+    order = np.lexsort((qq.reshape(-1), tot.reshape(-1)))[:100]
+    q, e = gpu_lowest(B, J, h, 100)
+    assert q.tolist() == qq.reshape(-1)[order].tolist()
+    np.testing.assert_allclose(e, tot.reshape(-1)[order], rtol=1e-13, atol=0)
+
+
+# ---------- the other entry points ----------
+def test_host_entry_point_and_energies(B):
+    import torch
+    c = I.baseline_config(1)
+    q, e = B.ising_lowest_host(c.J, c.h, c.S)
+    qo, eo = oracle.lowest(c.J, c.h, c.S)
+    assert_exact(q, e, qo, eo)
+    states = torch.from_numpy(np.arange(0, 5000, dtype=np.int64) * 199).cuda()
+    en = B.ising_energies(c.J, c.h, states).cpu().numpy()
+    np.testing.assert_array_equal(en, oracle.energies_of(c.J, c.h, states.cpu().numpy().astype(np.uint64)))
+
+
+def test_qubo_entry_point(B):
+    """eqs. (2),(3): F(q) = -sum a_ij q_i q_j - sum b_i q_i, brute force in numpy for N = 12."""
+    N = 12
+    rng = np.random.default_rng(12)
+    U = rng.standard_normal((N, N)); a = np.triu(U, 1) + np.triu(U, 1).T
+    b = rng.standard_normal(N)
+    X = ((np.arange(1 << N)[:, None] >> np.arange(N)[None, :]) & 1).astype(np.float64)
+    F = -np.einsum("qi,ij,qj->q", X, np.triu(a, 1), X) - X @ b
+    order = np.lexsort((np.arange(1 << N), F))[:50]
+    q, e = B.qubo_lowest(a, b, 50)
+    assert B.states_to_numpy(q).tolist() == order.tolist()
+    np.testing.assert_allclose(e.cpu().numpy(), F[order], rtol=1e-12, atol=1e-12)
+
+
+def test_error_codes_from_device_validation(B):
+    N = 16
+    J, h = I.complete_gaussian(N, seed=1)
+    bad = J.copy(); bad[2, 3] = np.nan; bad[3, 2] = np.nan
+    for Jx, hx, code in ((bad, h, B.ERR_NONFINITE),
+                         (J + np.eye(N), h, B.ERR_DIAGONAL),
+                         (J + np.triu(np.ones((N, N)), 1) * 1e-9, h, B.ERR_ASYMMETRIC),
+                         (J, np.where(np.arange(N) == 0, np.inf, h), B.ERR_NONFINITE)):
+        with pytest.raises(B.IsingError) as ei:
+            B.ising_lowest(Jx, hx, 4)
+        assert ei.value.status == code
+    with pytest.raises(B.IsingError) as ei:
+        B.ising_lowest(J, h, (1 << N) + 1)
+    assert ei.value.status == B.ERR_BAD_S
+
+
+def test_launch_shape_independence(B):
+    """The result must not depend on the walk length or the launch size (env knobs used for tuning)."""
+    c = I.baseline_config(2)
+    ref = gpu_lowest(B, c.J, c.h, c.S)
+    try:
+        for lw, ch in ((0, 28), (3, 30), (10, 44), (5, 24)):
+            os.environ["ISING_LW"] = str(lw); os.environ["ISING_CHUNK_LOG2"] = str(ch)
+            q, e = gpu_lowest(B, c.J, c.h, c.S)
+            assert q.tolist() == ref[0].tolist() and e.tolist() == ref[1].tolist()
+    finally:
+        os.environ.pop("ISING_LW", None); os.environ.pop("ISING_CHUNK_LOG2", None)
