@@ -1,0 +1,338 @@
+"""bench.py -- BASELINE.json metric on BASELINE.json configs[4]: the N=48 complete-graph Gaussian instance, S=100.
+
+A "step" is ONE full pass of the hot path over one instance: all 2^48 spin configurations enumerated, filtered,
+selected, the survivors re-evaluated in fp64 and the S lowest written.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config k] [--range-log2 r]
+
+  value        configurations evaluated per second, whole job, inputs resident in HBM, CUDA-event timed
+  e2e          same through ising_lowest_host: pinned HOST buffers in and out, copies inside the timed region
+  roofline     the enumeration kernel against the integer add-min ceiling
+  cpu_baseline the CPU oracle, as it stands, on a bounded prefix of the same instance (rank 0, N=1 only)
+
+N > 1 (torchrun): the path shards over independent problems -- one seeded instance per rank, no data-path
+collective -- so scaling is "weak" and value = N * 2^48 / (max over ranks of the device time).
+--impl reference times the CPU oracle (there is no other reference implementation in this tier).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "spin_configs_evaluated_per_s"
+UNIT = "configs/s"
+# integer-ALU ceiling of the inner operation (one VIADDMNMX per configuration), DESIGN.md "Roofline":
+# 148 SMs x 4 sub-partitions x 16 lanes/clk (ALU pipe, B300_MICROARCH.md "Pipe rates") x 1.965 GHz (MEASURED_PEAKS.json)
+ALU_LANES_PER_CLK_PER_SM = 64
+FMA_LANES_PER_CLK_PER_SM = 128
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=5, help="BASELINE.json config number (1-based); 5 = N=48")
+    ap.add_argument("--range-log2", type=int, default=0,
+                    help="development only: enumerate just the first 2^r states per step (0 = the whole space)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+def instance_for_rank(k: int, rank: int):
+    from paper_1904_03621_b200 import instances as I
+    c = I.baseline_config(k)
+    if rank == 0:
+        return c
+    # other ranks: an independent instance of the same ensemble (same generator, rank-specific seed)
+    if k in (1, 3, 5):
+        J, h = I.complete_gaussian(c.N, I.SEED_BASE + k + 1000 * rank, h_scale=0.5 if k == 3 else 1.0)
+        return I.Instance(f"{c.name}_rank{rank}", c.N, c.S, J, h, False)
+    return c
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region (B200_PROFILING.md recipe)."""
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.rows = []
+        self.proc = None
+        self.thread = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--query-gpu={self.FIELDS}", "--format=csv,noheader,nounits", "-lms", "200",
+                 "-i", str(self.index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except Exception:
+            self.proc = None
+            return
+        self.thread = threading.Thread(target=self._pump, daemon=True)
+        self.thread.start()
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.perf_counter(), line.strip()))
+
+    def stop(self):
+        if self.proc is not None:
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=5)
+            except Exception:
+                self.proc.kill()
+
+    def summary(self, t0: float, t1: float):
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for t, line in self.rows:
+            if t < t0 or t > t1:
+                continue
+            parts = [p.strip() for p in line.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                sm.append(float(parts[0])); mx.append(float(parts[1])); pw.append(float(parts[2]))
+            except ValueError:
+                continue
+            for name, val in zip(names, parts[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2], "sm_min_mhz": sm[0], "sm_max_mhz": max(mx), "power_w_max": max(pw),
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def oracle_sample_rate(inst, seconds_target: float, S: int):
+    """Time the oracle, as it stands, on a contiguous prefix of q sized for about `seconds_target` seconds."""
+    from oracle import oracle
+    cores = oracle.max_threads()
+    k = min(inst.N, 20)
+    t0 = time.perf_counter()
+    oracle.lowest(inst.J, inst.h, S, 0, 1 << k)
+    dt = max(time.perf_counter() - t0, 1e-6)
+    rate = (1 << k) / dt
+    want = rate * seconds_target
+    kk = k
+    while kk < inst.N and (1 << (kk + 1)) <= want:
+        kk += 1
+    if kk > k:
+        t0 = time.perf_counter()
+        oracle.lowest(inst.J, inst.h, S, 0, 1 << kk)
+        dt = time.perf_counter() - t0
+        rate = (1 << kk) / dt
+    return rate, cores, kk, dt
+
+
+def run_reference(args, rank: int, world: int):
+    """--impl reference: the CPU oracle on the box's host cores; each step is a bounded sample of the workload."""
+    if rank != 0:
+        return
+    from oracle import oracle
+    inst = instance_for_rank(args.config, 0)
+    cores = oracle.max_threads()
+    # size one step for roughly 3 s of oracle time
+    rate, _, kk, _ = oracle_sample_rate(inst, 3.0, inst.S)
+    n = 1 << kk
+    for _ in range(args.warmup):
+        oracle.lowest(inst.J, inst.h, inst.S, 0, n)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle.lowest(inst.J, inst.h, inst.S, 0, n)
+    dt = time.perf_counter() - t0
+    value = n * args.steps / dt
+    sample = (f"oracle.lowest on the first 2^{kk} of 2^{inst.N} states of {inst.name} per step; "
+              f"full-space time extrapolated = {float(1 << inst.N) / value:.3e} s")
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"BASELINE.json configs[{args.config - 1}]: {inst.name}, N={inst.N}, S={inst.S}",
+                   "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    args = parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+        return
+
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from paper_1904_03621_b200 import binding as B, build
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    if rank == 0:
+        build.build()
+    if world > 1:
+        dist.barrier()
+    B.load()
+
+    inst = instance_for_rank(args.config, rank)
+    N, S = inst.N, inst.S
+    q_end = 1 << N
+    if args.range_log2:
+        q_end = 1 << max(min(args.range_log2, N), min(N, 20))
+    configs_per_step = q_end
+    J = torch.from_numpy(inst.J).cuda()
+    h = torch.from_numpy(inst.h).cuda()
+    out = (torch.empty(S, dtype=torch.int64, device="cuda"), torch.empty(S, dtype=torch.float64, device="cuda"))
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")          # > 126 MB L2
+    stream = torch.cuda.current_stream()
+
+    def step():
+        B.ising_lowest_range(J, h, S, 0, q_end, stream=stream, out=out)
+        return B.last_stats()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # roofline denominators measured live on this device (also quoted: the nominal ones DESIGN.md derives)
+    fma_peak = B.fma_peak(50.0)
+    addmin_peak = B.addmin_peak(50.0)
+
+    for _ in range(args.warmup):
+        flush.zero_()
+        step()
+
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    time.sleep(0.3)
+    barrier()
+    t_wall0 = time.perf_counter()
+    dev_ms = 0.0
+    enum_ms = 0.0
+    enum_launches = 0
+    launches = 0
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    for _ in range(args.steps):
+        flush.zero_()                       # L2 flush between timed iterations (outside the event bracket)
+        ev0.record(stream)
+        st = step()
+        ev1.record(stream)
+        ev1.synchronize()
+        dev_ms += ev0.elapsed_time(ev1)
+        enum_ms += st.enum_ms
+        enum_launches += st.enum_launches
+        launches += st.kernel_launches
+    barrier()
+    t_wall1 = time.perf_counter()
+    clocks = sampler.summary(t_wall0, t_wall1)
+
+    # ---- end to end: pinned host buffers in, host buffers out, through ising_lowest_host ----
+    e2e = None
+    if not args.no_e2e:
+        Jh = torch.from_numpy(inst.J).pin_memory()
+        hh = torch.from_numpy(inst.h).pin_memory()
+        qh = torch.empty(S, dtype=torch.int64).pin_memory()
+        eh = torch.empty(S, dtype=torch.float64).pin_memory()
+        out_h = (qh.numpy().view(np.uint64), eh.numpy())
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            B.ising_lowest_host(Jh.numpy(), hh.numpy(), S, 0, q_end, stream=stream, out=out_h)
+        torch.cuda.synchronize()
+        e2e_s = time.perf_counter() - t0
+        assert qh.numpy().view(np.uint64).tolist() == B.states_to_numpy(out[0]).tolist()
+        e2e = {"seconds": e2e_s, "h2d": (N * N + N) * 8, "d2h": S * 16}
+    sampler.stop()
+
+    # max over ranks of the device time
+    times = torch.tensor([dev_ms, e2e["seconds"] if e2e else 0.0], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(times, op=dist.ReduceOp.MAX)
+    dev_ms_max, e2e_s_max = float(times[0]), float(times[1])
+    total_configs = float(configs_per_step) * args.steps * world
+    value = total_configs / (dev_ms_max * 1e-3)
+
+    if rank == 0:
+        sm_max_hz = 1.965e9
+        try:
+            peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+            sm_max_hz = float(peaks.get("sm_max_mhz", 1965.0)) * 1e6
+        except Exception:
+            pass
+        sms = torch.cuda.get_device_properties(local_rank).multi_processor_count
+        alu_peak = sms * ALU_LANES_PER_CLK_PER_SM * sm_max_hz          # add-min ops / s
+        fma_nominal = sms * FMA_LANES_PER_CLK_PER_SM * sm_max_hz       # FMA / s
+        achieved = float(configs_per_step) * args.steps / (enum_ms * 1e-3)   # one add-min per configuration
+        traffic = None
+        tpath = os.path.join(ROOT, "profiles", "enumerate_dram_bytes_per_launch.txt")
+        if os.path.exists(tpath):
+            try:
+                traffic = float(open(tpath).read().split()[0])
+            except Exception:
+                traffic = None
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": dev_ms_max / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "int32", "data": "synthetic",
+            "config": {"workload": f"BASELINE.json configs[{args.config - 1}]: {inst.name}, N={N}, S={S}, "
+                                   f"states [0, 2^{q_end.bit_length() - 1}) of 2^{N} per step",
+                       "parallelism": f"independent instances x{world}" if world > 1 else "single GPU",
+                       "l2": "256 MiB buffer written between timed steps (inputs are 18 KB; the path has no HBM traffic)",
+                       "grid_exponent_p": st.grid_exponent, "epsilon": st.epsilon, "kept": st.keep},
+            "time_to_S_lowest_s": dev_ms_max * 1e-3 / args.steps,
+            "fp32_fma_roofline": {"definition": "configs/s x N / peak FP32 FMA/s (BASELINE.json metric)",
+                                  "frac_of_measured": value / world * N / fma_peak,
+                                  "frac_of_nominal": value / world * N / fma_nominal,
+                                  "fma_per_s_measured": fma_peak, "fma_per_s_nominal": fma_nominal},
+            "roofline": {"bound": "alu", "achieved": achieved, "peak": alu_peak, "unit": "add-min/s",
+                         "frac": achieved / alu_peak, "traffic": traffic,
+                         "kernel": "ising::enumerate_kernel", "launches": enum_launches,
+                         "avg_launch_ms": enum_ms / max(enum_launches, 1),
+                         "peak_source": "derived: SMs x 64 ALU lanes/clk x sm_max_mhz of MEASURED_PEAKS.json",
+                         "peak_measured_live": addmin_peak, "frac_of_measured_live": achieved / addmin_peak},
+            "gpu_launches": launches,
+            "clocks": clocks,
+        }
+        if e2e:
+            line["e2e"] = {"value": total_configs / e2e_s_max, "unit": UNIT,
+                           "h2d_bytes_per_step": e2e["h2d"], "d2h_bytes_per_step": e2e["d2h"]}
+        if world == 1 and not args.no_cpu_baseline:
+            rate, cores, kk, dt = oracle_sample_rate(inst, 15.0, S)
+            line["cpu_baseline"] = {
+                "value": rate, "unit": UNIT, "cores": cores, "kind": "oracle",
+                "sample": f"oracle.lowest on the first 2^{kk} of 2^{N} states of {inst.name} ({dt:.1f} s); "
+                          f"full-space time extrapolated = {float(1 << N) / rate:.3e} s"}
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()
