@@ -129,6 +129,9 @@ typedef struct ising_stats {
     double   total_ms;           /* device time of the whole call */
     int32_t  keep;               /* K: candidates kept per list */
     int32_t  inner_bits;         /* L: unrolled Gray bits per inner block */
+    int32_t  kernel_variant;     /* 16: packed 16-bit screen + exact int32 re-forming of hit blocks (default);
+                                    32: int32 add-min per configuration (environment ISING_KERNEL=32) */
+    int32_t  screen_shift;       /* variant 16: one 16-bit unit = 2^screen_shift grid units (0: screen is exact) */
 } ising_stats;
 
 int ising_get_last_stats(ising_stats *out_host);

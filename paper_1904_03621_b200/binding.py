@@ -37,7 +37,8 @@ class _Stats(ctypes.Structure):
                 ("passes", ctypes.c_uint32), ("split_retries", ctypes.c_uint32),
                 ("grid_exponent", ctypes.c_int32), ("exact", ctypes.c_int32),
                 ("epsilon", ctypes.c_double), ("enum_ms", ctypes.c_double), ("total_ms", ctypes.c_double),
-                ("keep", ctypes.c_int32), ("inner_bits", ctypes.c_int32)]
+                ("keep", ctypes.c_int32), ("inner_bits", ctypes.c_int32),
+                ("kernel_variant", ctypes.c_int32), ("screen_shift", ctypes.c_int32)]
 
 
 @dataclass
@@ -55,6 +56,8 @@ class Stats:
     total_ms: float
     keep: int
     inner_bits: int
+    kernel_variant: int
+    screen_shift: int
 
 
 _lib = None
@@ -133,7 +136,7 @@ def last_stats() -> Stats:
     s = _Stats()
     _check(load().ising_get_last_stats(ctypes.byref(s)), "ising_get_last_stats")
     return Stats(s.configs, s.candidates, s.kernel_launches, s.enum_launches, s.passes, s.split_retries,
-                 s.grid_exponent, bool(s.exact), s.epsilon, s.enum_ms, s.total_ms, s.keep, s.inner_bits)
+                 s.grid_exponent, bool(s.exact), s.epsilon, s.enum_ms, s.total_ms, s.keep, s.inner_bits, s.kernel_variant, s.screen_shift)
 
 
 def ising_lowest_range(J, h, S: int, q_begin: int, q_end: int, stream=None, out=None):

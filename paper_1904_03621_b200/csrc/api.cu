@@ -102,6 +102,7 @@ int run_lowest(const double* J, const double* h, const double* Jorig, const doub
     memset(&stats, 0, sizeof(stats));
     const int lw_run = env_int("ISING_LW", 8, 0, LW_MAX);
     const int chunk_log2 = env_int("ISING_CHUNK_LOG2", 40, MIN_CHUNK_BITS, 44);
+    const int variant = env_int("ISING_KERNEL", 16, 16, 32) == 32 ? 32 : 16;   // 16: packed screen, 32: int32 kernel
 
     CUDA_TRY(cudaEventRecord(ws.ev[0], st));
     launch_stage(J, h, N, ws.tab, ws.ctrl, st, extra_eps_rel);
@@ -116,6 +117,8 @@ int run_lowest(const double* J, const double* h, const double* Jorig, const doub
     stats.exact = ws.h_ctrl->exact;
     stats.epsilon = ws.h_ctrl->epsilon;
     stats.inner_bits = LOWBITS;
+    stats.kernel_variant = variant;
+    stats.screen_shift = variant == 16 ? ws.h_ctrl->shift16 : -1;
     stats.passes = 1;
 
     double enum_ms = 0.0;
@@ -159,7 +162,8 @@ int run_lowest(const double* J, const double* h, const double* Jorig, const doub
                 cur += nt << (LOWBITS + Lw);
             }
             CUDA_TRY(cudaEventRecord(ws.ev[2], st));
-            launch_enumerate(ws.tab, ws.ctrl, ws.pool, N, pc.Lw, pc.base, pc.nthreads, st);
+            if (variant == 16) launch_enumerate16(ws.tab, ws.ctrl, ws.pool, N, pc.Lw, pc.base, pc.nthreads, st);
+            else launch_enumerate(ws.tab, ws.ctrl, ws.pool, N, pc.Lw, pc.base, pc.nthreads, st);
             CUDA_TRY(cudaEventRecord(ws.ev[3], st));
             stats.kernel_launches += 1;
             stats.enum_launches += 1;

@@ -72,7 +72,7 @@ struct Ctrl {
     unsigned count;        // entries in the pool (kept prefix + new candidates); may exceed POOL_CAP = overflow
     unsigned kept;         // entries of the sorted prefix after the last selection
     int tauE;              // filter threshold (grid units)
-    int pad0;
+    int shift16;           // copy of Tables::shift16 (written by tables_kernel) for the host's statistics
     unsigned long long tauQ;   // ties on tauE pass only for q < tauQ
     unsigned band_overflow;    // selection wanted to keep more than KEEP_CAP entries
     unsigned pad1;
@@ -89,6 +89,13 @@ struct Tables {
     int DV[LW_MAX * 2 * NLO];      // DV[k][sb][lo]  = sgn * -4 sum_{i in lo} Jq[i][w_k],  sgn = sb ? +1 : -1
     int DU[LW_MAX * 2 * NMID];     // DU[k][sb][mid] = sgn * -4 sum_{j in mid} Jq[j][w_k]
     int DW[1 << LW_MAX];           // DW[t] = -sgn_t * 4 sum_{j in R_t} Jq[w_k][w_j]   (walk-internal part of step t)
+    // ---- packed 16-bit screening tables of enumerate16.cu: two configurations per 32-bit word, in units of
+    //      2^shift16 grid units, every entry rounded DOWN (floor), so sums of them are lower bounds ----
+    int shift16;                   // s: one 16-bit unit = 2^s grid units (0 for small-integer instances: exact)
+    int cU16;                      // offset added to every 16-bit U entry so that it is never negative
+    unsigned Cp[(NMID / 2) * NLO]; // Cp[r][lo]  = pack( C[r][lo] >> s , C[r + 16][lo] >> s )   (low half, high half)
+    unsigned DVp[LW_MAX * 2 * NLO];        // DVp[k][sb][lo] = +-(DV[k][1][lo] >> s) * 65537    (both halves alike)
+    unsigned DUp[LW_MAX * 2 * (NMID / 2)]; // DUp[k][sb][r]  = +-((DU[k][1][r] >> s) + 65536 (DU[k][1][r + 16] >> s))
 };
 
 struct Geometry {
@@ -105,6 +112,9 @@ void launch_qubo_to_ising(const double* a, const double* b, int N, double* J, do
 void launch_enumerate(const Tables* tab, Ctrl* ctrl, Entry* pool, int N, int Lw,
                       unsigned long long base, unsigned nthreads, cudaStream_t st);
 void launch_direct(const Tables* tab, Ctrl* ctrl, Entry* pool, int N, cudaStream_t st);
+// enumerate16.cu
+void launch_enumerate16(const Tables* tab, Ctrl* ctrl, Entry* pool, int N, int Lw,
+                        unsigned long long base, unsigned nthreads, cudaStream_t st);
 // select.cu
 int  launch_select(Entry* pool, Ctrl* ctrl, unsigned n, int S, cudaStream_t st);     // returns kernels launched
 int  launch_final(const double* J, const double* h, int N, int mode, Entry* pool, unsigned m, int S,

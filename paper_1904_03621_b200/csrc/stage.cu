@@ -129,7 +129,7 @@ __global__ void __launch_bounds__(256) stage_kernel(const double* __restrict__ J
 }
 
 // Tables of the QUBO form relative to the base state (see file header). One block; thread-per-entry loops.
-__global__ void __launch_bounds__(256) tables_kernel(Tables* __restrict__ tab, const Ctrl* __restrict__ ctrl, int N)
+__global__ void __launch_bounds__(256) tables_kernel(Tables* __restrict__ tab, Ctrl* __restrict__ ctrl, int N)
 {
     if (ctrl->status != ISING_OK) return;
     const int tid = threadIdx.x;
@@ -176,6 +176,64 @@ __global__ void __launch_bounds__(256) tables_kernel(Tables* __restrict__ tab, c
             v = -sgn * 4 * acc;
         }
         tab->DW[t] = v;
+    }
+
+    // ---- packed 16-bit screening tables (enumerate16.cu). One 16-bit unit = 2^s grid units; every entry is
+    // floored, so V16 + C16 + U16 <= (V + C + U) / 2^s: a rigorous lower bound of the block energy.
+    // Range: |Phi_i| <= R_i = |hq_i| + sum_j |Jq_ij| for every state, hence
+    //   |V| <= BV = max|QL| + 2 sum_{i in lo} R_i,  |U| <= BU = max|QM| + 2 sum_{i in mid} R_i,  |C| <= BC = max|C|.
+    // A quantised entry is off by less than 1 unit, a walked table by less than 1 + LW_MAX units (one floor per
+    // set walk bit). s is the smallest shift for which no 16-bit lane can wrap (see enumerate16.cu header):
+    //   X16 = (BX >> s) + 2 + LW_MAX,   cU = U16,   V16 + C16 + 2 cU <= 32767.
+    __shared__ int s_shift, s_cU;
+    __syncthreads();                                   // QL, QM, C above are complete
+    if (tid == 0) {
+        long long BV = 0, BU = 0, BC = 0, m;
+        for (int x = 0; x < NLO; ++x) { m = tab->QL[x]; m = m < 0 ? -m : m; if (m > BV) BV = m; }
+        for (int x = 0; x < NMID; ++x) { m = tab->QM[x]; m = m < 0 ? -m : m; if (m > BU) BU = m; }
+        for (int x = 0; x < NMID * NLO; ++x) { m = tab->C[x]; m = m < 0 ? -m : m; if (m > BC) BC = m; }
+        for (int i = 0; i < LOWBITS && i < N; ++i) {
+            long long R = tab->hq[i] < 0 ? -(long long)tab->hq[i] : tab->hq[i];
+            for (int j = 0; j < N; ++j) { m = Jq[i * 64 + j]; R += m < 0 ? -m : m; }
+            if (i < LL) BV += 2 * R; else BU += 2 * R;
+        }
+        int s = 0;
+        for (; s < 40; ++s) {
+            const long long V16 = (BV >> s) + 2 + LW_MAX, U16 = (BU >> s) + 2 + LW_MAX, C16 = (BC >> s) + 2;
+            if (V16 + C16 + 2 * U16 <= 32767) break;
+        }
+        s_shift = s;
+        s_cU = (int)((BU >> s) + 2 + LW_MAX);
+        tab->shift16 = s;
+        tab->cU16 = s_cU;
+        ctrl->shift16 = s;
+    }
+    __syncthreads();
+    const int s16 = s_shift;
+    for (int idx = tid; idx < (NMID / 2) * NLO; idx += blockDim.x) {
+        const int r = idx / NLO, lo = idx % NLO;
+        const int a = tab->C[r * NLO + lo] >> s16, b = tab->C[(r + NMID / 2) * NLO + lo] >> s16;
+        tab->Cp[idx] = ((unsigned)a & 0xffffu) | ((unsigned)b << 16);
+    }
+    for (int idx = tid; idx < LW_MAX * NLO; idx += blockDim.x) {
+        const int k = idx / NLO, lo = idx % NLO;
+        int acc = 0;
+        for (int i = 0; i < LL; ++i) if (lo >> i & 1) acc += Jat(i, LOWBITS + k);
+        const int d = (-4 * acc) >> s16;               // = DV[k][1][lo] >> s : the bit turns on
+        tab->DVp[(k * 2 + 1) * NLO + lo] = (unsigned)(d * 65537);
+        tab->DVp[(k * 2 + 0) * NLO + lo] = (unsigned)(-d * 65537);
+    }
+    for (int idx = tid; idx < LW_MAX * (NMID / 2); idx += blockDim.x) {
+        const int k = idx / (NMID / 2), r = idx % (NMID / 2);
+        int acc0 = 0, acc1 = 0;
+        for (int j = 0; j < LM; ++j) {
+            if (r >> j & 1) acc0 += Jat(LL + j, LOWBITS + k);
+            if ((r + NMID / 2) >> j & 1) acc1 += Jat(LL + j, LOWBITS + k);
+        }
+        const int d0 = (-4 * acc0) >> s16, d1 = (-4 * acc1) >> s16;
+        const int D = d0 + 65536 * d1;                 // integer sum: halves never wrap (biased, non-negative)
+        tab->DUp[(k * 2 + 1) * (NMID / 2) + r] = (unsigned)D;
+        tab->DUp[(k * 2 + 0) * (NMID / 2) + r] = (unsigned)(-D);
     }
 }
 
