@@ -180,6 +180,7 @@ enumerate16_kernel(const Tables* __restrict__ tab, Ctrl* __restrict__ ctrl, Entr
 
     const unsigned nsteps = 1u << Lw;
     for (unsigned t = 0; t < nsteps; ++t) {
+        asm volatile("" ::: "memory");                 // the tables are re-read every step: keep them out of registers
         if (t > 0) {
             // ---- Gray step: flip walk bit k = ctz(t); warp-uniform rows; packed words updated on the FMA pipe ----
             const int k = __ffs(t) - 1;
