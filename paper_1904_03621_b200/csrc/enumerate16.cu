@@ -143,7 +143,7 @@ enumerate16_kernel(const Tables* __restrict__ tab, Ctrl* __restrict__ ctrl, Entr
 
     const int s16 = tab->shift16;
     const int cU = tab->cU16;
-    unsigned Vp[NLO], Up[NHALF];
+    unsigned Va[NLO], Vb[NLO], Up[NHALF];
     {
         // exact V[x] = QL[x] - 2 sum_{i in x} Phi_i by subset sums, then floor to 16-bit units and bias
         int acc[NLO];
@@ -155,8 +155,9 @@ enumerate16_kernel(const Tables* __restrict__ tab, Ctrl* __restrict__ ctrl, Entr
         }
 #pragma unroll
         for (int x = 0; x < NLO; ++x) {
-            const unsigned vb = (unsigned)(((acc[x] + tab->QL[x]) >> s16) + 32768);
-            Vp[x] = vb * 65537u;
+            const int v = acc[x] + tab->QL[x];
+            Va[x] = (unsigned)((v >> s16) + 32768) * 65537u;                           // mid bit 4 clear
+            Vb[x] = (unsigned)(((v + tab->C[16 * NLO + x]) >> s16) + 32768) * 65537u;  // mid bit 4 set
         }
         acc[0] = 0;
 #pragma unroll
@@ -166,8 +167,9 @@ enumerate16_kernel(const Tables* __restrict__ tab, Ctrl* __restrict__ ctrl, Entr
         }
 #pragma unroll
         for (int r = 0; r < NHALF; ++r) {
-            const unsigned u0 = (unsigned)(((acc[r] + tab->QM[r]) >> s16) + cU);
-            const unsigned u1 = (unsigned)(((acc[r + NHALF] + tab->QM[r + NHALF]) >> s16) + cU);
+            const int m0 = (r & 7) | ((r >> 3) << 4), m1 = m0 | 8;
+            const unsigned u0 = (unsigned)(((acc[m0] + tab->QM[m0]) >> s16) + cU);
+            const unsigned u1 = (unsigned)(((acc[m1] + tab->QM[m1]) >> s16) + cU);
             Up[r] = u0 + (u1 << 16);
         }
     }
@@ -193,10 +195,14 @@ enumerate16_kernel(const Tables* __restrict__ tab, Ctrl* __restrict__ ctrl, Entr
 #pragma unroll
             for (int x = 0; x < NLO / 4; ++x) {
                 const uint4 d = dv[x];
-                Vp[4 * x + 0] = add_fma_pipe(Vp[4 * x + 0], d.x);
-                Vp[4 * x + 1] = add_fma_pipe(Vp[4 * x + 1], d.y);
-                Vp[4 * x + 2] = add_fma_pipe(Vp[4 * x + 2], d.z);
-                Vp[4 * x + 3] = add_fma_pipe(Vp[4 * x + 3], d.w);
+                Va[4 * x + 0] = add_fma_pipe(Va[4 * x + 0], d.x);
+                Va[4 * x + 1] = add_fma_pipe(Va[4 * x + 1], d.y);
+                Va[4 * x + 2] = add_fma_pipe(Va[4 * x + 2], d.z);
+                Va[4 * x + 3] = add_fma_pipe(Va[4 * x + 3], d.w);
+                Vb[4 * x + 0] = add_fma_pipe(Vb[4 * x + 0], d.x);
+                Vb[4 * x + 1] = add_fma_pipe(Vb[4 * x + 1], d.y);
+                Vb[4 * x + 2] = add_fma_pipe(Vb[4 * x + 2], d.z);
+                Vb[4 * x + 3] = add_fma_pipe(Vb[4 * x + 3], d.w);
             }
 #pragma unroll
             for (int x = 0; x < NHALF / 4; ++x) {
@@ -210,18 +216,25 @@ enumerate16_kernel(const Tables* __restrict__ tab, Ctrl* __restrict__ ctrl, Entr
         // ---- a3: 1024 configurations, one packed add-min per two of them ----
         unsigned g = 0xffffffffu;
 #pragma unroll
-        for (int r = 0; r < NHALF; ++r) {
+        for (int r = 0; r < NHALF / 2; ++r) {
+            // one row of C serves two register sets (mid bit 4 clear / set): 8 add-mins per LDS.128,
+            // and the two chains are independent
             const uint4* crow = reinterpret_cast<const uint4*>(sCp + r * NLO);
-            unsigned m = 0xffffffffu;
+            unsigned ma = 0xffffffffu, mb = 0xffffffffu;
 #pragma unroll
             for (int x = 0; x < NLO / 4; ++x) {
                 const uint4 c = crow[x];
-                m = __viaddmin_u16x2(Vp[4 * x + 0], c.x, m);
-                m = __viaddmin_u16x2(Vp[4 * x + 1], c.y, m);
-                m = __viaddmin_u16x2(Vp[4 * x + 2], c.z, m);
-                m = __viaddmin_u16x2(Vp[4 * x + 3], c.w, m);
+                ma = __viaddmin_u16x2(Va[4 * x + 0], c.x, ma);
+                mb = __viaddmin_u16x2(Vb[4 * x + 0], c.x, mb);
+                ma = __viaddmin_u16x2(Va[4 * x + 1], c.y, ma);
+                mb = __viaddmin_u16x2(Vb[4 * x + 1], c.y, mb);
+                ma = __viaddmin_u16x2(Va[4 * x + 2], c.z, ma);
+                mb = __viaddmin_u16x2(Vb[4 * x + 2], c.z, mb);
+                ma = __viaddmin_u16x2(Va[4 * x + 3], c.w, ma);
+                mb = __viaddmin_u16x2(Vb[4 * x + 3], c.w, mb);
             }
-            g = __viaddmin_u16x2(m, Up[r], g);
+            g = __viaddmin_u16x2(ma, Up[r], g);
+            g = __viaddmin_u16x2(mb, Up[r + NHALF / 2], g);
         }
         // ---- a4: threshold filter on the lower bound:  bound * 2^s + Eh <= tauE  <=>  bound <= (tauE - Eh) >> s ----
         const int gm = (int)min(g & 0xffffu, g >> 16) - bias;

@@ -210,9 +210,12 @@ __global__ void __launch_bounds__(256) tables_kernel(Tables* __restrict__ tab, C
     }
     __syncthreads();
     const int s16 = s_shift;
+    // pairing: the two halves of a packed word differ in mid bit 3 (spin LL + 3); u = 0..15 runs over the other four
+    // mid bits, mid0(u) = (u & 7) | ((u >> 3) << 4). Rows u < 8 have mid bit 4 clear, rows u >= 8 have it set.
     for (int idx = tid; idx < (NMID / 2) * NLO; idx += blockDim.x) {
-        const int r = idx / NLO, lo = idx % NLO;
-        const int a = tab->C[r * NLO + lo] >> s16, b = tab->C[(r + NMID / 2) * NLO + lo] >> s16;
+        const int u = idx / NLO, lo = idx % NLO;
+        const int m0 = (u & 7) | ((u >> 3) << 4);
+        const int a = tab->C[m0 * NLO + lo] >> s16, b = tab->C[(m0 | 8) * NLO + lo] >> s16;
         tab->Cp[idx] = ((unsigned)a & 0xffffu) | ((unsigned)b << 16);
     }
     for (int idx = tid; idx < LW_MAX * NLO; idx += blockDim.x) {
@@ -225,10 +228,11 @@ __global__ void __launch_bounds__(256) tables_kernel(Tables* __restrict__ tab, C
     }
     for (int idx = tid; idx < LW_MAX * (NMID / 2); idx += blockDim.x) {
         const int k = idx / (NMID / 2), r = idx % (NMID / 2);
+        const int m0 = (r & 7) | ((r >> 3) << 4), m1 = m0 | 8;
         int acc0 = 0, acc1 = 0;
         for (int j = 0; j < LM; ++j) {
-            if (r >> j & 1) acc0 += Jat(LL + j, LOWBITS + k);
-            if ((r + NMID / 2) >> j & 1) acc1 += Jat(LL + j, LOWBITS + k);
+            if (m0 >> j & 1) acc0 += Jat(LL + j, LOWBITS + k);
+            if (m1 >> j & 1) acc1 += Jat(LL + j, LOWBITS + k);
         }
         const int d0 = (-4 * acc0) >> s16, d1 = (-4 * acc1) >> s16;
         const int D = d0 + 65536 * d1;                 // integer sum: halves never wrap (biased, non-negative)
