@@ -30,8 +30,10 @@ if ROOT not in sys.path:
 
 METRIC = "spin_configs_evaluated_per_s"
 UNIT = "configs/s"
-# integer-ALU ceiling of the inner operation (one VIADDMNMX per configuration), DESIGN.md "Roofline":
-# 148 SMs x 4 sub-partitions x 16 lanes/clk (ALU pipe, B300_MICROARCH.md "Pipe rates") x 1.965 GHz (MEASURED_PEAKS.json)
+# integer-ALU ceiling of the inner operation: VIADDMNMX issues on the ALU pipe at
+# 148 SMs x 4 sub-partitions x 16 lanes/clk (B300_MICROARCH.md "Pipe rates") x 1.965 GHz (MEASURED_PEAKS.json);
+# the default kernel's VIADDMNMX.U16x2 forms two 16-bit add-mins (two configurations) per lane instruction,
+# the int32 kernel (ISING_KERNEL=32) one.
 ALU_LANES_PER_CLK_PER_SM = 64
 FMA_LANES_PER_CLK_PER_SM = 128
 
@@ -223,6 +225,7 @@ def main():
     # roofline denominators measured live on this device (also quoted: the nominal ones DESIGN.md derives)
     fma_peak = B.fma_peak(50.0)
     addmin_peak = B.addmin_peak(50.0)
+    addmin16x2_peak = B.addmin16x2_peak(50.0)
 
     for _ in range(args.warmup):
         flush.zero_()
@@ -286,7 +289,10 @@ def main():
         except Exception:
             pass
         sms = torch.cuda.get_device_properties(local_rank).multi_processor_count
-        alu_peak = sms * ALU_LANES_PER_CLK_PER_SM * sm_max_hz          # add-min ops / s
+        per_inst = 2 if st.kernel_variant == 16 else 1                 # add-mins (configurations) per lane instruction
+        alu_peak = sms * ALU_LANES_PER_CLK_PER_SM * sm_max_hz * per_inst          # add-min ops / s
+        live_peak = addmin16x2_peak * 2 if st.kernel_variant == 16 else addmin_peak
+        kname = "ising::enumerate16_kernel" if st.kernel_variant == 16 else "ising::enumerate_kernel"
         fma_nominal = sms * FMA_LANES_PER_CLK_PER_SM * sm_max_hz       # FMA / s
         achieved = float(configs_per_step) * args.steps / (enum_ms * 1e-3)   # one add-min per configuration
         traffic = None
@@ -299,12 +305,16 @@ def main():
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": dev_ms_max / args.steps, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "int32", "data": "synthetic",
+            "scaling": "weak", "vs_baseline": None,
+            "dtype": "int16x2 screen + int32 exact (fp64 output)" if st.kernel_variant == 16 else "int32 (fp64 output)",
+            "data": "synthetic",
             "config": {"workload": f"BASELINE.json configs[{args.config - 1}]: {inst.name}, N={N}, S={S}, "
                                    f"states [0, 2^{q_end.bit_length() - 1}) of 2^{N} per step",
                        "parallelism": f"independent instances x{world}" if world > 1 else "single GPU",
                        "l2": "256 MiB buffer written between timed steps (inputs are 18 KB; the path has no HBM traffic)",
-                       "grid_exponent_p": st.grid_exponent, "epsilon": st.epsilon, "kept": st.keep},
+                       "grid_exponent_p": st.grid_exponent, "epsilon": st.epsilon, "kept": st.keep,
+                       "kernel_variant": st.kernel_variant, "screen_shift": st.screen_shift,
+                       "candidates": st.candidates},
             "time_to_S_lowest_s": dev_ms_max * 1e-3 / args.steps,
             "fp32_fma_roofline": {"definition": "configs/s x N / peak FP32 FMA/s (BASELINE.json metric)",
                                   "frac_of_measured": value / world * N / fma_peak,
@@ -312,10 +322,12 @@ def main():
                                   "fma_per_s_measured": fma_peak, "fma_per_s_nominal": fma_nominal},
             "roofline": {"bound": "alu", "achieved": achieved, "peak": alu_peak, "unit": "add-min/s",
                          "frac": achieved / alu_peak, "traffic": traffic,
-                         "kernel": "ising::enumerate_kernel", "launches": enum_launches,
+                         "kernel": kname, "launches": enum_launches,
                          "avg_launch_ms": enum_ms / max(enum_launches, 1),
-                         "peak_source": "derived: SMs x 64 ALU lanes/clk x sm_max_mhz of MEASURED_PEAKS.json",
-                         "peak_measured_live": addmin_peak, "frac_of_measured_live": achieved / addmin_peak},
+                         "peak_source": f"derived: SMs x 64 ALU lanes/clk x {per_inst} add-min per lane instruction "
+                                        "x sm_max_mhz of MEASURED_PEAKS.json (DESIGN.md 5.2)",
+                         "peak_measured_live": live_peak, "frac_of_measured_live": achieved / live_peak,
+                         "viaddmnmx_s32_per_s_live": addmin_peak, "viaddmnmx_u16x2_per_s_live": addmin16x2_peak},
             "gpu_launches": launches,
             "clocks": clocks,
         }

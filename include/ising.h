@@ -149,6 +149,11 @@ int ising_fma_peak(double ms_target, double *fma_per_s_out_host, void *stream);
  * (DESIGN.md "Roofline"). */
 int ising_addmin_peak(double ms_target, double *addmin_per_s_out_host, void *stream);
 
+/* Same for the packed inner operation of the default kernel (SASS VIADDMNMX.U16x2): lane INSTRUCTIONS per second,
+ * whole GPU; each instruction forms two 16-bit add-mins, i.e. screens two configurations, so the configuration
+ * ceiling of the packed kernel is twice this number. */
+int ising_addmin16x2_peak(double ms_target, double *inst_per_s_out_host, void *stream);
+
 /* Frees the calling thread's cached workspace (device pool, tables, pinned control block). Optional. */
 void ising_release_workspace(void);
 

@@ -22,7 +22,7 @@ S_MAX = 65536
 # every symbol include/ising.h declares (tests/test_abi.py checks the header against this list and the .so)
 EXPORTS = ["ising_lowest", "ising_lowest_range", "ising_lowest_host", "ising_merge_lists", "qubo_lowest",
            "ising_energies", "ising_get_last_stats", "ising_strerror", "ising_last_error", "ising_version",
-           "ising_fma_peak", "ising_addmin_peak", "ising_release_workspace"]
+           "ising_fma_peak", "ising_addmin_peak", "ising_addmin16x2_peak", "ising_release_workspace"]
 
 
 class IsingError(RuntimeError):
@@ -87,8 +87,10 @@ def load():
     lib.ising_get_last_stats.argtypes = [ctypes.POINTER(_Stats)]
     lib.ising_fma_peak.argtypes = [ctypes.c_double, ctypes.POINTER(ctypes.c_double), vp]
     lib.ising_addmin_peak.argtypes = [ctypes.c_double, ctypes.POINTER(ctypes.c_double), vp]
+    lib.ising_addmin16x2_peak.argtypes = [ctypes.c_double, ctypes.POINTER(ctypes.c_double), vp]
     for name in ("ising_lowest", "ising_lowest_range", "ising_lowest_host", "ising_merge_lists", "qubo_lowest",
-                 "ising_energies", "ising_get_last_stats", "ising_fma_peak", "ising_addmin_peak", "ising_version"):
+                 "ising_energies", "ising_get_last_stats", "ising_fma_peak", "ising_addmin_peak", "ising_addmin16x2_peak",
+                 "ising_version"):
         getattr(lib, name).restype = ctypes.c_int
     lib.ising_strerror.argtypes = [ctypes.c_int]
     lib.ising_strerror.restype = ctypes.c_char_p
@@ -247,6 +249,13 @@ def fma_peak(ms_target: float = 50.0, stream=None) -> float:
 def addmin_peak(ms_target: float = 50.0, stream=None) -> float:
     v = ctypes.c_double(0.0)
     _check(load().ising_addmin_peak(float(ms_target), ctypes.byref(v), _stream(stream)), "ising_addmin_peak")
+    return v.value
+
+
+def addmin16x2_peak(ms_target: float = 50.0, stream=None) -> float:
+    """VIADDMNMX.U16x2 lane instructions per second (two 16-bit add-mins each)."""
+    v = ctypes.c_double(0.0)
+    _check(load().ising_addmin16x2_peak(float(ms_target), ctypes.byref(v), _stream(stream)), "ising_addmin16x2_peak")
     return v.value
 
 

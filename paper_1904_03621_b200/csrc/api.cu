@@ -100,8 +100,8 @@ int run_lowest(const double* J, const double* h, const double* Jorig, const doub
     Workspace& ws = t_ws;
     ising_stats stats;
     memset(&stats, 0, sizeof(stats));
-    const int lw_run = env_int("ISING_LW", 8, 0, LW_MAX);
-    const int chunk_log2 = env_int("ISING_CHUNK_LOG2", 40, MIN_CHUNK_BITS, 44);
+    const int lw_run = env_int("ISING_LW", LW_MAX, 0, LW_MAX);
+    const int chunk_log2 = env_int("ISING_CHUNK_LOG2", 42, MIN_CHUNK_BITS, 44);
     const int variant = env_int("ISING_KERNEL", 16, 16, 32) == 32 ? 32 : 16;   // 16: packed screen, 32: int32 kernel
 
     CUDA_TRY(cudaEventRecord(ws.ev[0], st));
@@ -391,6 +391,15 @@ int ising_addmin_peak(double ms_target, double* addmin_per_s_out_host, void* str
     double r = run_fma_peak(ms_target, (cudaStream_t)stream, 1);
     if (r < 0.0) { t_last_error = "VIADDMNMX microbenchmark failed"; return ISING_ERR_CUDA; }
     *addmin_per_s_out_host = r;
+    return ISING_OK;
+}
+
+int ising_addmin16x2_peak(double ms_target, double* inst_per_s_out_host, void* stream)
+{
+    if (!inst_per_s_out_host) return ISING_ERR_NULL;
+    double r = run_fma_peak(ms_target, (cudaStream_t)stream, 2);
+    if (r < 0.0) { t_last_error = "VIADDMNMX.U16x2 microbenchmark failed"; return ISING_ERR_CUDA; }
+    *inst_per_s_out_host = r;
     return ISING_OK;
 }
 

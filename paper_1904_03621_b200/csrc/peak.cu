@@ -1,6 +1,7 @@
 // peak.cu -- roofline denominators measured on the device the library runs on (build step 1).
 //   which = 0 : FP32 FFMA      (lane-FMAs per second, the BASELINE.json "FP32 FMA roofline")
-//   which = 1 : VIADDMNMX.S32  (lane add-min per second: the integer-ALU ceiling of the enumeration's inner op)
+//   which = 1 : VIADDMNMX.S32  (lane add-min per second: the integer-ALU ceiling of the int32 kernel's inner op)
+//   which = 2 : VIADDMNMX.U16x2 (lane instructions per second; each one is TWO 16-bit add-mins: enumerate16.cu)
 // Each thread runs 8 independent dependency chains, 16 deep per loop trip; nothing touches memory inside the loop.
 #include "common.cuh"
 
@@ -19,7 +20,8 @@ __global__ void __launch_bounds__(256) peak_kernel(int iters, float fa, float fb
 #pragma unroll
             for (int c = 0; c < 8; ++c) {
                 if (WHICH == 0) f[c] = fmaf(f[c], fa, fb);
-                else v[c] = __viaddmin_s32(v[c], ia, ib);
+                else if (WHICH == 1) v[c] = __viaddmin_s32(v[c], ia, ib);
+                else v[c] = (int)__viaddmin_u16x2((unsigned)v[c], (unsigned)ia, (unsigned)ib);
             }
         }
     }
@@ -43,7 +45,8 @@ double run_fma_peak(double ms_target, cudaStream_t st, int which)
     const int blocks = sms * 8, threads = 256;
     auto launch = [&](int iters) {
         if (which == 0) peak_kernel<0><<<blocks, threads, 0, st>>>(iters, 0.999f, 0.001f, 1, 1 << 30, sink);
-        else peak_kernel<1><<<blocks, threads, 0, st>>>(iters, 0.999f, 0.001f, 1, 1 << 30, sink);
+        else if (which == 1) peak_kernel<1><<<blocks, threads, 0, st>>>(iters, 0.999f, 0.001f, 1, 1 << 30, sink);
+        else peak_kernel<2><<<blocks, threads, 0, st>>>(iters, 0.999f, 0.001f, 0x00010001, 0x7fff7fff, sink);
     };
     auto timed = [&](int iters) -> double {
         cudaEventRecord(e0, st);

@@ -59,6 +59,26 @@ __global__ void __launch_bounds__(256) stage_kernel(const double* __restrict__ J
         __syncthreads();
     }
     const double W = s_red[0];
+    // smallest exponent p_req with every weight an integer multiple of 2^-p_req (the instance's own grid):
+    // x = M 2^(e-53), M a 53-bit integer  =>  lowest set bit of x has exponent e - 53 + ctz(M)
+    __shared__ int s_preq;
+    if (tid == 0) s_preq = -100000;
+    __syncthreads();
+    {
+        int req = -100000;
+        for (int idx = tid; idx < N * N + N; idx += blockDim.x) {
+            const double v = idx < N * N ? J[idx] : h[idx - N * N];
+            if (v != 0.0 && isfinite(v)) {
+                int e;
+                const double m = frexp(fabs(v), &e);
+                const unsigned long long M = (unsigned long long)ldexp(m, 53);
+                const int low = e - 53 + (__ffsll((long long)M) - 1);
+                if (-low > req) req = -low;
+            }
+        }
+        if (req > -100000) atomicMax(&s_preq, req);
+    }
+    __syncthreads();
     if (tid == 0) {
         int p = 0, st = ISING_OK;
         if (!isfinite(W)) st = ISING_ERR_RANGE_W;
@@ -67,6 +87,8 @@ __global__ void __launch_bounds__(256) stage_kernel(const double* __restrict__ J
             frexp(W * (1.0 + 1e-9), &e);          // W < 2^e  (the factor covers the rounding of the fp64 sum)
             p = WQ_BITS - e;                      // sum of |rint(x 2^p)| <= W 2^p + (#terms)/2 < 2^27 + 2^11
             if (p > 1000 || p < -1000) st = ISING_ERR_RANGE_W;
+            // integer / dyadic instance whose own grid fits: use it (smaller integers, exact and a finer 16-bit screen)
+            else if (s_preq <= p && s_preq >= -1000) p = s_preq;
         }
         s_p = p;
         s_status = st;

@@ -312,3 +312,131 @@ def test_launch_shape_independence(B):
             assert q.tolist() == ref[0].tolist() and e.tolist() == ref[1].tolist()
     finally:
         os.environ.pop("ISING_LW", None); os.environ.pop("ISING_CHUNK_LOG2", None)
+
+
+# ---------- the two enumeration kernels (packed 16-bit screen = default, int32 = ISING_KERNEL=32) ----------
+def _with_kernel(variant, fn):
+    os.environ["ISING_KERNEL"] = str(variant)
+    try:
+        return fn()
+    finally:
+        os.environ.pop("ISING_KERNEL", None)
+
+
+def _wide_range_instance(N, seed):
+    """Weights spanning six decades: the 16-bit screen is coarse (large shift), false hits are frequent."""
+    rng = np.random.default_rng(seed)
+    U = rng.standard_normal((N, N)) * 10.0 ** rng.uniform(-3, 3, size=(N, N))
+    J = np.triu(U, 1) + np.triu(U, 1).T
+    h = rng.standard_normal(N) * 10.0 ** rng.uniform(-3, 3, size=N)
+    return J, h
+
+
+@pytest.mark.parametrize("name", ["cfg1", "cfg2", "int22", "wide21", "bigint20", "range36"])
+def test_kernel_variants_agree_with_oracle(B, name):
+    q_begin = q_end = None
+    if name == "cfg1":
+        c = I.baseline_config(1); J, h, S = c.J, c.h, c.S
+    elif name == "cfg2":
+        c = I.baseline_config(2); J, h, S = c.J, c.h, c.S
+    elif name == "int22":
+        J, h = I.random_integer(22, seed=2222, wmax=3, density=0.6); S = 500
+    elif name == "wide21":
+        J, h = _wide_range_instance(21, 77); S = 200
+    elif name == "bigint20":
+        # integer weights up to 10^5: exact mode (epsilon = 0) but a coarse 16-bit screen (shift > 0)
+        rng = np.random.default_rng(20)
+        U = rng.integers(-100000, 100001, size=(20, 20)).astype(np.float64)
+        J = np.triu(U, 1) + np.triu(U, 1).T
+        h = rng.integers(-100000, 100001, size=20).astype(np.float64); S = 300
+    else:
+        c = I.baseline_config(3); J, h, S = c.J, c.h, c.S
+        q_begin, q_end = 5 << 30, (5 << 30) + (3 << 21)
+    res = {}
+    for v in (16, 32):
+        res[v] = _with_kernel(v, lambda: gpu_lowest(B, J, h, S, q_begin, q_end))
+        st = B.last_stats()
+        assert st.kernel_variant == v
+        if v == 16 and name == "bigint20":
+            assert st.exact and st.screen_shift > 0
+        if v == 16 and name == "cfg2":
+            assert st.exact and st.screen_shift == 0
+    assert res[16][0].tolist() == res[32][0].tolist() and res[16][1].tolist() == res[32][1].tolist()
+    if name == "cfg2":
+        return                                            # 2^32 states: the stored golden covers it
+    qo, eo = oracle.lowest(J, h, S) if q_begin is None else oracle.lowest(J, h, S, q_begin, q_end)
+    assert_exact(res[16][0], res[16][1], qo, eo)
+
+
+# ---------- N = 48 at full size: closed forms and constructions the oracle can reach (SURVEY.md P7, P8, P10, P11) ----------
+def test_mattis_48_full_space(B):
+    """P7: gauge-transformed ferromagnet, J_ij = xi_i xi_j, integer, 2^48 states: ground pair, then the 96 one-flip
+    states in q order (E depends only on the number of spins that disagree with xi)."""
+    N = 48
+    full = (1 << N) - 1
+    J, h, xi = I.mattis(N, seed=4848)
+    q_xi = sum(1 << i for i in range(N) if xi[i] > 0)
+    E0 = -N * (N - 1) / 2
+    E1 = -((N - 2) ** 2 - N) / 2
+    exp = [(E0, q_xi), (E0, full ^ q_xi)]
+    exp += [(E1, q_xi ^ (1 << i)) for i in range(N)] + [(E1, full ^ q_xi ^ (1 << i)) for i in range(N)]
+    exp = sorted(exp)
+    q, e = gpu_lowest(B, J, h, len(exp))
+    st = B.last_stats()
+    assert st.exact and st.configs == 1 << N
+    assert [(float(ee), int(qq)) for qq, ee in zip(q, e)] == exp
+
+
+def test_two_blocks_48_pair_sums(B):
+    """P8: two decoupled 24-spin Gaussian blocks; the oracle enumerates each block (2 x 2^24), the lowest states of
+    the 48-spin instance are the smallest pair sums. Real weights: exercises the guard band at 48 bits."""
+    NA = NB = 24
+    J, h = I.two_blocks(NA, NB, seed=4824)
+    eA = oracle.energies_range(J[:NA, :NA], h[:NA], 0, 1 << NA)
+    eB = oracle.energies_range(J[NA:, NA:], h[NA:], 0, 1 << NB)
+    K = 400
+    ia = np.argsort(eA, kind="stable")[:K]; ib = np.argsort(eB, kind="stable")[:K]
+    tot = eA[ia][None, :] + eB[ib][:, None]
+    qq = ia[None, :].astype(np.uint64) | (ib[:, None].astype(np.uint64) << np.uint64(NA))
+    S = 100
+    order = np.lexsort((qq.reshape(-1), tot.reshape(-1)))[:S]
+    assert tot.reshape(-1)[order][-1] < eA[ia[-1]] + eB[ib[0]]      # K was large enough: nothing outside can enter
+    q, e = gpu_lowest(B, J, h, S)
+    assert B.last_stats().configs == 1 << 48
+    assert q.tolist() == qq.reshape(-1)[order].tolist()
+    np.testing.assert_allclose(e, tot.reshape(-1)[order], rtol=1e-12, atol=0)
+    np.testing.assert_array_equal(oracle.energies_of(J, h, q), e)   # and bit-exact against eq. (1) state by state
+
+
+def test_config5_full_run_properties(B):
+    """cfg5 (N = 48 complete Gaussian), where no complete oracle run exists: necessary conditions (P11) and the
+    gauge metamorphic relation (P10) on the full 2^48 space."""
+    c = I.baseline_config(5)
+    q, e = gpu_lowest(B, c.J, c.h, c.S)
+    st = B.last_stats()
+    assert st.configs == 1 << c.N and not st.exact
+    np.testing.assert_array_equal(oracle.energies_of(c.J, c.h, q), e)
+    pairs = list(zip(e.tolist(), q.tolist()))
+    assert pairs == sorted(pairs) and len(set(q.tolist())) == c.S
+    _neighbour_check(c.J, c.h, q, e, nflip=2)
+    rng = np.random.default_rng(5)
+    g = 2.0 * rng.integers(0, 2, size=c.N) - 1.0
+    mask = np.uint64(sum(1 << i for i in range(c.N) if g[i] < 0))
+    q2, e2 = gpu_lowest(B, c.J * np.outer(g, g), c.h * g, c.S)
+    assert (q2 ^ mask).tolist() == q.tolist()
+    np.testing.assert_allclose(e2, e, rtol=1e-12, atol=0)
+
+
+def test_sharded_single_rank_gpu(B):
+    """sharded.ising_lowest_sharded with no process group = the plain call; plus the rank loop run serially."""
+    import torch
+    from paper_1904_03621_b200 import sharded
+    c = I.baseline_config(1)
+    q, e = sharded.ising_lowest_sharded(c.J, c.h, c.S)
+    qo, eo = oracle.lowest(c.J, c.h, c.S)
+    assert_exact(B.states_to_numpy(q), e.cpu().numpy(), qo, eo)
+    c = I.baseline_config(3)
+    full = B.ising_lowest(c.J, c.h, c.S)
+    parts = [B.ising_lowest_range(c.J, c.h, c.S, a, b) for a, b in sharded.shard_ranges(c.N, 8)]
+    qm, em = B.ising_merge_lists(torch.cat([p[0] for p in parts]), torch.cat([p[1] for p in parts]), c.S)
+    assert torch.equal(qm, full[0]) and torch.equal(em, full[1])
