@@ -334,6 +334,29 @@ def main():
         if e2e:
             line["e2e"] = {"value": total_configs / e2e_s_max, "unit": UNIT,
                            "h2d_bytes_per_step": e2e["h2d"], "d2h_bytes_per_step": e2e["d2h"]}
+        if world == 1 and not args.range_log2:
+            # north_star: configs/s and time-to-solution for every BASELINE.json config (the other four are
+            # parity-test cases, reported here for reference only: median of 5 whole-space calls, CUDA events)
+            per = []
+            for k in (1, 2, 3, 4):
+                ck = instance_for_rank(k, 0)
+                Jk = torch.from_numpy(ck.J).cuda(); hk = torch.from_numpy(ck.h).cuda()
+                ts = []
+                for _ in range(6):
+                    ev0.record(stream)
+                    B.ising_lowest(Jk, hk, ck.S, stream=stream)
+                    ev1.record(stream); ev1.synchronize()
+                    ts.append(ev0.elapsed_time(ev1))
+                ms = sorted(ts[1:])[2]
+                stk = B.last_stats()
+                per.append({"config": k, "name": ck.name, "N": ck.N, "S": ck.S, "time_to_S_lowest_ms": ms,
+                            "configs_per_s": float(1 << ck.N) / (ms * 1e-3), "exact": bool(stk.exact),
+                            "screen_shift": stk.screen_shift, "candidates": stk.candidates,
+                            "fp32_fma_roofline_frac": float(1 << ck.N) / (ms * 1e-3) * ck.N / fma_peak})
+            per.append({"config": 5, "name": inst.name, "N": N, "S": S, "time_to_S_lowest_ms": dev_ms_max / args.steps,
+                        "configs_per_s": value, "exact": bool(st.exact), "screen_shift": st.screen_shift,
+                        "candidates": st.candidates, "fp32_fma_roofline_frac": value * N / fma_peak})
+            line["per_config"] = per
         if world == 1 and not args.no_cpu_baseline:
             rate, cores, kk, dt = oracle_sample_rate(inst, 15.0, S)
             line["cpu_baseline"] = {

@@ -94,5 +94,50 @@ def lowest(J, h, S: int, q_begin: int = 0, q_end: int | None = None, threads: in
     return states[:n].copy(), en[:n].copy()
 
 
+_SO_GRAY = os.path.join(_HERE, "liboracle_gray.so")
+_lib_gray = None
+
+
+def build_gray(force: bool = False) -> str:
+    """Compile oracle_gray.c (tier-2 oracle for integer instances; see its header)."""
+    src = os.path.join(_HERE, "oracle_gray.c")
+    if force or not os.path.exists(_SO_GRAY) or os.path.getmtime(_SO_GRAY) < os.path.getmtime(src):
+        subprocess.check_call(["gcc", "-O2", "-fopenmp", "-fPIC", "-shared", "-o", _SO_GRAY, src, "-lm"])
+    return _SO_GRAY
+
+
+def lowest_gray(J, h, S: int, q_begin: int = 0, q_end: int | None = None, slab_bits: int | None = None,
+                threads: int = 0):
+    """Tier-2 oracle (single-spin-flip recurrence in exact int64), INTEGER-weight instances only.
+    Pinned to `lowest` by tests/test_oracle_pins.py; used to write tests/golden/cfg4.txt."""
+    global _lib_gray
+    if _lib_gray is None:
+        build_gray()
+        lib = ctypes.CDLL(_SO_GRAY)
+        dp = ctypes.POINTER(ctypes.c_double)
+        up = ctypes.POINTER(ctypes.c_uint64)
+        lib.oracle_gray_lowest.restype = ctypes.c_int64
+        lib.oracle_gray_lowest.argtypes = [dp, dp, ctypes.c_int, ctypes.c_int64, ctypes.c_uint64, ctypes.c_uint64,
+                                           ctypes.c_int, up, dp, ctypes.c_int]
+        _lib_gray = lib
+    J, h, N, Jp, hp = _prep(J, h)
+    if q_end is None:
+        q_end = 1 << N
+    if slab_bits is None:
+        slab_bits = min(N, 22)
+        while (q_begin | q_end) & ((1 << slab_bits) - 1):
+            slab_bits -= 1
+    states = np.empty(S, dtype=np.uint64)
+    en = np.empty(S, dtype=np.float64)
+    n = _lib_gray.oracle_gray_lowest(Jp, hp, N, int(S), int(q_begin), int(q_end), int(slab_bits),
+                                     states.ctypes.data_as(ctypes.POINTER(ctypes.c_uint64)),
+                                     en.ctypes.data_as(ctypes.POINTER(ctypes.c_double)), int(threads))
+    if n == -2:
+        raise ValueError("oracle_gray_lowest: integer weights only")
+    if n < 0:
+        raise ValueError("oracle_gray_lowest: bad arguments")
+    return states[:n].copy(), en[:n].copy()
+
+
 def max_threads() -> int:
     return int(_load().oracle_max_threads())

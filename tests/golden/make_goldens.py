@@ -5,8 +5,11 @@ Usage:  python tests/golden/make_goldens.py [config numbers ...]     (default: 1
 
 Each file cfg<k>.txt holds the oracle's S+16 lowest (q, E) pairs of BASELINE.json config k
 (energy as a C99 hex float, so the file is bit-exact), plus the instance SHA-256. Config 1 takes
-under a second, config 2 minutes, config 3 about two hours on 8 cores; configs 4 and 5 are out of
-reach of the plain oracle.
+under a second, config 2 minutes, config 3 about 2.6 hours on 8 cores with the plain oracle (oracle.c).
+Config 4 (2^40 states, integer weights) is out of reach of the plain oracle (about 40 hours) and is written
+by the tier-2 oracle oracle_gray.c (exact int64 single-spin-flip recurrence, pinned to oracle.c by
+tests/test_oracle_pins.py) in about half an hour; its file says so. Config 5 is out of reach of both
+(DESIGN.md "Parity status").
 With --chunks C the state space is cut into C equal ranges of q; the oracle's S+16 lowest of each range
 (oracle_lowest on [q_begin, q_end)) are appended to tests/golden/.cfg<k>.partial as they finish, so an
 interrupted run resumes where it stopped; the union of the per-range lists is then ordered by (E, q) and cut
@@ -48,7 +51,8 @@ def lowest_chunked(c, k, chunks):
         if i in done:
             continue
         t0 = time.time()
-        q, e = oracle.lowest(c.J, c.h, min(c.S + EXTRA, step), i * step, (i + 1) * step)
+        solve = oracle.lowest_gray if k == 4 else oracle.lowest
+        q, e = solve(c.J, c.h, min(c.S + EXTRA, step), i * step, (i + 1) * step)
         dt = time.time() - t0
         with open(part, "a") as f:
             for qq, ee in zip(q, e):
@@ -73,12 +77,13 @@ def main(argv):
         if chunks:
             q, e, dt = lowest_chunked(c, k, chunks)
         else:
-            q, e = oracle.lowest(c.J, c.h, c.S + EXTRA)
+            q, e = (oracle.lowest_gray if k == 4 else oracle.lowest)(c.J, c.h, c.S + EXTRA)
             dt = time.time() - t0
         path = os.path.join(HERE, f"cfg{k}.txt")
         with open(path, "w") as f:
             f.write(f"# BASELINE.json config {k}: {c.name}, N={c.N}, S={c.S} (+{EXTRA} spare)\n")
-            f.write(f"# written by tests/golden/make_goldens.py from oracle/oracle.c only; oracle wall time {dt:.1f} s, "
+            src = "oracle/oracle_gray.c (tier-2 oracle, integer instances)" if k == 4 else "oracle/oracle.c"
+            f.write(f"# written by tests/golden/make_goldens.py from {src} only; oracle wall time {dt:.1f} s, "
                     f"{oracle.max_threads()} threads\n")
             f.write(f"# instance sha256 {c.sha256()}\n")
             for qq, ee in zip(q, e):

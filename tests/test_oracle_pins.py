@@ -203,3 +203,45 @@ def test_bad_arguments():
         oracle.lowest(J, h, 0)
     with pytest.raises(ValueError):
         oracle.lowest(J, h, 4, 0, 1 << 5)
+
+
+# ---------- tier-2 oracle (oracle_gray.c, integer instances only) pinned to the plain oracle ----------
+@pytest.mark.parametrize("N,wmax,density,S", [(3, 1, 1.0, 8), (8, 3, 1.0, 256), (13, 2, 0.4, 500), (17, 1, 0.2, 1000),
+                                              (20, 3, 0.3, 2000), (22, 5, 0.15, 300)])
+def test_gray_oracle_equals_plain_oracle(N, wmax, density, S):
+    J, h = I.random_integer(N, seed=31 * N + wmax, wmax=wmax, density=density)
+    qo, eo = oracle.lowest(J, h, S)
+    for slab in sorted({0, 1, min(N, 5), min(N, 11), N}):
+        qg, eg = oracle.lowest_gray(J, h, S, slab_bits=slab)
+        assert qg.tolist() == qo.tolist() and eg.tolist() == eo.tolist()
+
+
+def test_gray_oracle_ranges_threads_and_closed_form():
+    J, h = I.random_integer(18, seed=99, wmax=2, density=0.5)
+    lo, hi = 3 << 14, 11 << 14
+    qo, eo = oracle.lowest(J, h, 700, lo, hi)
+    for threads in (1, 3):
+        qg, eg = oracle.lowest_gray(J, h, 700, lo, hi, slab_bits=12, threads=threads)
+        assert qg.tolist() == qo.tolist() and eg.tolist() == eo.tolist()
+    # Mattis closed form at a size the plain oracle does not reach quickly (N = 30): ground pair + 2N one-flip states
+    N = 30
+    J, h, xi = I.mattis(N, seed=7)
+    q_xi = sum(1 << i for i in range(N) if xi[i] > 0)
+    full = (1 << N) - 1
+    E0 = -N * (N - 1) / 2
+    E1 = -((N - 2) ** 2 - N) / 2
+    exp = sorted([(E0, q_xi), (E0, full ^ q_xi)] + [(E1, q_xi ^ (1 << i)) for i in range(N)]
+                 + [(E1, full ^ q_xi ^ (1 << i)) for i in range(N)])
+    qg, eg = oracle.lowest_gray(J, h, len(exp))
+    assert [(float(e), int(q)) for q, e in zip(qg, eg)] == exp
+    with pytest.raises(ValueError):
+        oracle.lowest_gray(J + 0.5 * (1 - np.eye(N)), h, 4)          # non-integer weights are refused
+
+
+def test_gray_oracle_reproduces_config2_golden(golden_dir):
+    """Config 2's stored list was written by the PLAIN oracle (358 s); the tier-2 oracle must reproduce it exactly."""
+    from checker import load_golden
+    c = I.baseline_config(2)
+    qo, eo = load_golden(os.path.join(golden_dir, "cfg2.txt"))
+    qg, eg = oracle.lowest_gray(c.J, c.h, len(qo), threads=2)
+    assert qg.tolist() == qo.tolist() and eg.tolist() == eo.tolist()
