@@ -240,6 +240,36 @@ def ising_energies(J, h, states, stream=None):
     return out
 
 
+@dataclass
+class Solution:
+    """What the paper's `search` returns (Listing 1): energies and states, lowest first."""
+    energies: "object"      # numpy float64 [num_states]
+    states: "object"        # numpy uint64 [num_states]; bit i-1 of a state <-> the paper's 1-based spin i
+
+
+def search(graph: dict, num_states: int = 1, stream=None) -> Solution:
+    """The paper's one-call interface (Listing 1): `graph` maps 1-based index pairs to weights,
+    (i, j) with i != j is the coupling J_ij of eq. (1) and (i, i) is the field h_i. Marshalling only:
+    the dict is laid out as dense (J, h) and handed to `ising_lowest`; (i, j) and (j, i) must not both be given."""
+    import numpy as np
+    if not graph:
+        raise ValueError("empty graph")
+    N = max(max(i, j) for i, j in graph)
+    if min(min(i, j) for i, j in graph) < 1:
+        raise ValueError("spin indices are 1-based (PAPER.md:137)")
+    J = np.zeros((N, N), dtype=np.float64)
+    h = np.zeros(N, dtype=np.float64)
+    for (i, j), w in graph.items():
+        if i == j:
+            h[i - 1] = w
+        else:
+            if (j, i) in graph:
+                raise ValueError(f"both ({i},{j}) and ({j},{i}) given")
+            J[i - 1, j - 1] = J[j - 1, i - 1] = w
+    q, e = ising_lowest(J, h, int(num_states), stream=stream)
+    return Solution(energies=e.cpu().numpy(), states=states_to_numpy(q))
+
+
 def fma_peak(ms_target: float = 50.0, stream=None) -> float:
     v = ctypes.c_double(0.0)
     _check(load().ising_fma_peak(float(ms_target), ctypes.byref(v), _stream(stream)), "ising_fma_peak")

@@ -138,7 +138,7 @@ def test_config1_golden(B, golden_dir):
     assert_real(q, e, qo, eo, np.abs(np.triu(c.J, 1)).sum() + np.abs(c.h).sum(), c.S)
 
 
-@pytest.mark.parametrize("k", [2, 3])
+@pytest.mark.parametrize("k", [2, 3, 4])
 def test_config_golden(B, golden_dir, k):
     path = os.path.join(golden_dir, f"cfg{k}.txt")
     if not os.path.exists(path):
@@ -440,3 +440,13 @@ def test_sharded_single_rank_gpu(B):
     parts = [B.ising_lowest_range(c.J, c.h, c.S, a, b) for a, b in sharded.shard_ranges(c.N, 8)]
     qm, em = B.ising_merge_lists(torch.cat([p[0] for p in parts]), torch.cat([p[1] for p in parts]), c.S)
     assert torch.equal(qm, full[0]) and torch.equal(em, full[1])
+
+
+def test_search_sugar_listing1(B, golden_dir):
+    """The paper's Listing 1 through the paper-style `search(graph, num_states)` call."""
+    rows = [l.split() for l in open(os.path.join(golden_dir, "listing1.txt")) if l.strip() and l[0] != "#"]
+    sol = B.search({(1, 1): -1, (1, 2): -0.2}, num_states=4)
+    assert sol.states.tolist() == [int(r[0]) for r in rows]
+    np.testing.assert_allclose(sol.energies, [float(r[1]) for r in rows], rtol=0, atol=1e-15)
+    with pytest.raises(ValueError):
+        B.search({(1, 2): 1.0, (2, 1): 1.0}, 1)
