@@ -450,3 +450,15 @@ def test_search_sugar_listing1(B, golden_dir):
     np.testing.assert_allclose(sol.energies, [float(r[1]) for r in rows], rtol=0, atol=1e-15)
     with pytest.raises(ValueError):
         B.search({(1, 2): 1.0, (2, 1): 1.0}, 1)
+
+
+@pytest.mark.parametrize("N,seed", [(50, 50), (56, 56), (63, 63)])
+def test_subrange_parity_beyond_48(B, N, seed):
+    """include/ising.h accepts N <= 63: ranges near the top of the 2^N space (bits up to 62 set in q)."""
+    J, h = I.complete_gaussian(N, seed=seed)
+    top = (1 << N) >> 20
+    for lo_unit, units in ((top - 3, 3), (top // 3, 2)):
+        lo, hi = lo_unit << 20, (lo_unit + units) << 20
+        q, e = gpu_lowest(B, J, h, 64, lo, hi)
+        qo, eo = oracle.lowest(J, h, 64, lo, hi)
+        assert_exact(q, e, qo, eo)
