@@ -96,6 +96,16 @@ int ising_merge_lists(const uint64_t *states_in_dev, const double *energies_in_d
                       uint64_t *states_out_dev, double *energies_out_dev, void *stream);
 
 /*
+ * ising_lowest_h0 -- zero-field instances (h = 0), using the global spin-flip symmetry E(q) = E(~q) of eq. (1)
+ * (SURVEY.md section 8(f) item 3): only the half space q < 2^(N-1) is enumerated, every kept state brings its
+ * complement (same fp64 energy) with it, and the 2 S candidates are ordered by (energy, q) and cut at S.
+ * The result equals ising_lowest(J, 0, N, S) element for element; ising_stats.configs reports the 2^(N-1)
+ * configurations actually evaluated (half the space: an EFFECTIVE rate must not be quoted as configs/s evaluated).
+ * For N <= 20 the whole space is enumerated. J_dev as in ising_lowest.
+ */
+int ising_lowest_h0(const double *J_dev, int N, int S, uint64_t *states_out_dev, double *energies_out_dev, void *stream);
+
+/*
  * qubo_lowest -- QUBO entry point, eqs. (2),(3):
  *      F(q) = - sum_{i<j} a_ij q_i q_j - sum_i b_i q_i ,   q_i in {0,1}
  * a_dev [N*N] symmetric zero-diagonal, b_dev [N]. Converted on the device to the equivalent Ising

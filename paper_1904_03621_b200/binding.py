@@ -20,7 +20,7 @@ N_MAX = 63
 S_MAX = 65536
 
 # every symbol include/ising.h declares (tests/test_abi.py checks the header against this list and the .so)
-EXPORTS = ["ising_lowest", "ising_lowest_range", "ising_lowest_host", "ising_merge_lists", "qubo_lowest",
+EXPORTS = ["ising_lowest", "ising_lowest_range", "ising_lowest_host", "ising_lowest_h0", "ising_merge_lists", "qubo_lowest",
            "ising_energies", "ising_get_last_stats", "ising_strerror", "ising_last_error", "ising_version",
            "ising_fma_peak", "ising_addmin_peak", "ising_addmin16x2_peak", "ising_release_workspace"]
 
@@ -82,6 +82,8 @@ def load():
     lib.ising_lowest_range.argtypes = [dp, dp, i32, i32, u64, u64, up, dp, vp]
     lib.ising_lowest_host.argtypes = [dp, dp, i32, i32, u64, u64, up, dp, vp]
     lib.ising_merge_lists.argtypes = [up, dp, i64, i32, up, dp, vp]
+    lib.ising_lowest_h0.argtypes = [dp, i32, i32, up, dp, vp]
+    lib.ising_lowest_h0.restype = ctypes.c_int
     lib.qubo_lowest.argtypes = [dp, dp, i32, i32, up, dp, vp]
     lib.ising_energies.argtypes = [dp, dp, i32, up, i64, dp, vp]
     lib.ising_get_last_stats.argtypes = [ctypes.POINTER(_Stats)]
@@ -173,6 +175,19 @@ def ising_lowest(J, h, S: int, stream=None, out=None):
         rc = load().ising_lowest(J.data_ptr(), h.data_ptr(), N, int(S), states.data_ptr(), energies.data_ptr(),
                                  _stream(stream))
     _check(rc, "ising_lowest")
+    return states, energies
+
+
+def ising_lowest_h0(J, S: int, stream=None):
+    """Zero-field instance: half-space enumeration + complements (include/ising.h)."""
+    import torch
+    N = len(J)
+    J = _dev_f64(J, (N, N))
+    states = torch.empty(S, dtype=torch.int64, device=J.device)
+    energies = torch.empty(S, dtype=torch.float64, device=J.device)
+    with torch.cuda.device(J.device):
+        rc = load().ising_lowest_h0(J.data_ptr(), N, int(S), states.data_ptr(), energies.data_ptr(), _stream(stream))
+    _check(rc, "ising_lowest_h0")
     return states, energies
 
 

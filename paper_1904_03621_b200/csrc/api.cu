@@ -295,6 +295,31 @@ int ising_lowest_host(const double* J_host, const double* h_host, int N, int S, 
     return ISING_OK;
 }
 
+int ising_lowest_h0(const double* J_dev, int N, int S, uint64_t* states_out_dev, double* energies_out_dev, void* stream)
+{
+    t_last_error.clear();
+    if (N < 1 || N > ISING_N_MAX) { t_last_error = "N out of range"; return ISING_ERR_BAD_N; }
+    int rc = check_args(J_dev, J_dev, N, S, 0, 1ull << N, states_out_dev, energies_out_dev);
+    if (rc != ISING_OK) return rc;
+    rc = ensure_workspace();
+    if (rc != ISING_OK) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    Workspace& ws = t_ws;
+    CUDA_TRY(cudaMemsetAsync(ws.h2, 0, sizeof(double) * 64, st));
+    if (N <= 20)      // too small for a half-space range (ranges are multiples of 2^min(N,20)): plain call
+        return run_lowest(J_dev, ws.h2, nullptr, nullptr, 0, 0.0, N, S, 0, 1ull << N,
+                          (unsigned long long*)states_out_dev, energies_out_dev, st);
+    const unsigned long long half = 1ull << (N - 1);
+    const int S_half = (unsigned long long)S < half ? S : (int)half;
+    rc = run_lowest(J_dev, ws.h2, nullptr, nullptr, 0, 0.0, N, S_half, 0, half, ws.out_q, ws.out_e, st);
+    if (rc != ISING_OK) return rc;
+    t_stats.kernel_launches += launch_expand_complements(ws.out_q, ws.out_e, S_half, N, S, ws.pool,
+                                                         (unsigned long long*)states_out_dev, energies_out_dev, st);
+    CUDA_TRY(cudaStreamSynchronize(st));
+    CUDA_TRY(cudaGetLastError());
+    return ISING_OK;
+}
+
 int qubo_lowest(const double* a_dev, const double* b_dev, int N, int S, uint64_t* states_out_dev,
                 double* energies_out_dev, void* stream)
 {

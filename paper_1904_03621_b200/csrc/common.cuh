@@ -123,6 +123,8 @@ void launch_energies(const double* J, const double* h, int N, int mode, const un
                      long long n, double* out, cudaStream_t st);
 int  launch_merge_lists(const unsigned long long* states, const double* energies, long long n, int S, Entry* scratch,
                         unsigned long long* states_out, double* energies_out, cudaStream_t st);
+int  launch_expand_complements(const unsigned long long* states, const double* energies, int n, int N, int S,
+                               Entry* scratch, unsigned long long* states_out, double* energies_out, cudaStream_t st);
 // peak.cu
 double run_fma_peak(double ms_target, cudaStream_t st, int which);
 

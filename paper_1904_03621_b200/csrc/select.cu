@@ -258,6 +258,30 @@ __global__ void pack_kernel(const unsigned long long* __restrict__ states, const
     scratch[i] = e;
 }
 
+// h = 0: E(q) = E(~q). Every kept state of the lower half space brings its complement (same energy) with it.
+__global__ void expand_complement_kernel(const unsigned long long* __restrict__ states, const double* __restrict__ energies,
+                                         int n, unsigned long long mask, Entry* __restrict__ scratch)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    Entry e;
+    e.key = key_from_f64(energies[i]);
+    e.q = states[i];
+    scratch[2 * i] = e;
+    e.q = ~states[i] & mask;
+    scratch[2 * i + 1] = e;
+}
+
+int launch_expand_complements(const unsigned long long* states, const double* energies, int n, int N, int S,
+                              Entry* scratch, unsigned long long* states_out, double* energies_out, cudaStream_t st)
+{
+    const unsigned long long mask = N >= 64 ? ~0ull : ((1ull << N) - 1ull);
+    expand_complement_kernel<<<(n + 255) / 256, 256, 0, st>>>(states, energies, n, mask, scratch);
+    int launches = 1 + sort_pool(scratch, 2u * (unsigned)n, st);
+    emit_kernel<<<(S + 255) / 256, 256, 0, st>>>(scratch, S, states_out, energies_out);
+    return launches + 1;
+}
+
 int launch_merge_lists(const unsigned long long* states, const double* energies, long long n, int S, Entry* scratch,
                        unsigned long long* states_out, double* energies_out, cudaStream_t st)
 {

@@ -462,3 +462,21 @@ def test_subrange_parity_beyond_48(B, N, seed):
         q, e = gpu_lowest(B, J, h, 64, lo, hi)
         qo, eo = oracle.lowest(J, h, 64, lo, hi)
         assert_exact(q, e, qo, eo)
+
+
+def test_zero_field_symmetry_entry_point(B):
+    """ising_lowest_h0 (half-space enumeration + complements) = ising_lowest(J, 0): element for element."""
+    import torch
+    cases = [(I.baseline_config(2).J, 100), (I.complete_gaussian(26, seed=26)[0], 333), (I.mattis(33, seed=3)[0], 70),
+             (I.complete_gaussian(10, seed=10)[0], 1 << 10), (I.complete_gaussian(21, seed=21)[0], 1 << 16)]
+    for J, S in cases:
+        N = len(J)
+        q0, e0 = B.ising_lowest(J, np.zeros(N), S)
+        full_configs = B.last_stats().configs
+        q1, e1 = B.ising_lowest_h0(J, S)
+        assert torch.equal(q0, q1) and torch.equal(e0, e1)
+        assert B.last_stats().configs == (full_configs if N <= 20 else full_configs // 2)
+    c = I.baseline_config(2)
+    qo, eo = load_golden(os.path.join(os.path.dirname(__file__), "golden", "cfg2.txt"))
+    q1, e1 = B.ising_lowest_h0(c.J, c.S)
+    assert_exact(B.states_to_numpy(q1), e1.cpu().numpy(), qo[:c.S], eo[:c.S])
