@@ -357,6 +357,18 @@ def main():
                         "configs_per_s": value, "exact": bool(st.exact), "screen_shift": st.screen_shift,
                         "candidates": st.candidates, "fp32_fma_roofline_frac": value * N / fma_peak})
             line["per_config"] = per
+            # the paper's own pipeline (Algorithm 1) written plainly for this GPU, on a 2^28-state slice of the same
+            # instance: the on-box "prior design" figure; not a target, not the reference arm
+            n_alg1 = 1 << min(28, N)
+            B.ising_lowest_alg1(J, h, S, 0, n_alg1, stream=stream)
+            ev0.record(stream)
+            B.ising_lowest_alg1(J, h, S, 0, n_alg1, stream=stream)
+            ev1.record(stream); ev1.synchronize()
+            line["paper_pipeline_on_box"] = {
+                "value": float(n_alg1) / (ev0.elapsed_time(ev1) * 1e-3), "unit": UNIT,
+                "what": "ising_lowest_alg1: chunks of 2^20 states, eq. (1) directly in fp64 per state, chunk stored, "
+                        "S lowest selected by a full sort (PAPER.md:91-114)",
+                "sample": f"first 2^{n_alg1.bit_length() - 1} states of {inst.name}"}
         if world == 1 and not args.no_cpu_baseline:
             rate, cores, kk, dt = oracle_sample_rate(inst, 15.0, S)
             line["cpu_baseline"] = {

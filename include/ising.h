@@ -96,6 +96,18 @@ int ising_merge_lists(const uint64_t *states_in_dev, const double *energies_in_d
                       uint64_t *states_out_dev, double *energies_out_dev, void *stream);
 
 /*
+ * ising_lowest_alg1 -- the PAPER'S OWN pipeline (Algorithm 1), written plainly for this GPU, as the
+ * on-box comparison for the design above: the range is cut into chunks of
+ * 2^chunk_log2 states (10 <= chunk_log2 <= 20); every state's energy is evaluated directly by eq. (1) in fp64,
+ * O(N^2) per state, the chunk is stored in device memory behind the S lowest found so far
+ * (low_en / low_st) and the S lowest of the two are selected by a full sort. No Gray walk, no
+ * tables, no threshold filter, no grid or guard band: an independent exact path, several thousand times slower.
+ * Same arguments, result, order and error codes as ising_lowest_range.
+ */
+int ising_lowest_alg1(const double *J_dev, const double *h_dev, int N, int S, uint64_t q_begin, uint64_t q_end,
+                      int chunk_log2, uint64_t *states_out_dev, double *energies_out_dev, void *stream);
+
+/*
  * ising_lowest_h0 -- zero-field instances (h = 0), using the global spin-flip symmetry E(q) = E(~q) of eq. (1)
  * (SURVEY.md section 8(f) item 3): only the half space q < 2^(N-1) is enumerated, every kept state brings its
  * complement (same fp64 energy) with it, and the 2 S candidates are ordered by (energy, q) and cut at S.
@@ -139,7 +151,7 @@ typedef struct ising_stats {
     double   total_ms;           /* device time of the whole call */
     int32_t  keep;               /* K: candidates kept per list */
     int32_t  inner_bits;         /* L: unrolled Gray bits per inner block */
-    int32_t  kernel_variant;     /* 16: packed 16-bit screen + exact int32 re-forming of hit blocks (default);
+    int32_t  kernel_variant;     /* 1: ising_lowest_alg1. 16: packed 16-bit screen + exact int32 re-forming of hit blocks (default);
                                     32: int32 add-min per configuration (environment ISING_KERNEL=32) */
     int32_t  screen_shift;       /* variant 16: one 16-bit unit = 2^screen_shift grid units (0: screen is exact) */
 } ising_stats;

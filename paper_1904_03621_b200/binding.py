@@ -20,7 +20,7 @@ N_MAX = 63
 S_MAX = 65536
 
 # every symbol include/ising.h declares (tests/test_abi.py checks the header against this list and the .so)
-EXPORTS = ["ising_lowest", "ising_lowest_range", "ising_lowest_host", "ising_lowest_h0", "ising_merge_lists", "qubo_lowest",
+EXPORTS = ["ising_lowest", "ising_lowest_range", "ising_lowest_host", "ising_lowest_h0", "ising_lowest_alg1", "ising_merge_lists", "qubo_lowest",
            "ising_energies", "ising_get_last_stats", "ising_strerror", "ising_last_error", "ising_version",
            "ising_fma_peak", "ising_addmin_peak", "ising_addmin16x2_peak", "ising_release_workspace"]
 
@@ -83,6 +83,8 @@ def load():
     lib.ising_lowest_host.argtypes = [dp, dp, i32, i32, u64, u64, up, dp, vp]
     lib.ising_merge_lists.argtypes = [up, dp, i64, i32, up, dp, vp]
     lib.ising_lowest_h0.argtypes = [dp, i32, i32, up, dp, vp]
+    lib.ising_lowest_alg1.argtypes = [dp, dp, i32, i32, u64, u64, i32, up, dp, vp]
+    lib.ising_lowest_alg1.restype = ctypes.c_int
     lib.ising_lowest_h0.restype = ctypes.c_int
     lib.qubo_lowest.argtypes = [dp, dp, i32, i32, up, dp, vp]
     lib.ising_energies.argtypes = [dp, dp, i32, up, i64, dp, vp]
@@ -175,6 +177,23 @@ def ising_lowest(J, h, S: int, stream=None, out=None):
         rc = load().ising_lowest(J.data_ptr(), h.data_ptr(), N, int(S), states.data_ptr(), energies.data_ptr(),
                                  _stream(stream))
     _check(rc, "ising_lowest")
+    return states, energies
+
+
+def ising_lowest_alg1(J, h, S: int, q_begin: int = 0, q_end: int | None = None, chunk_log2: int = 20, stream=None):
+    """The paper's Algorithm 1 written plainly (include/ising.h): direct fp64 energies per chunk + full-sort selection."""
+    import torch
+    h = _dev_f64(h, (len(h),))
+    N = h.shape[0]
+    J = _dev_f64(J, (N, N))
+    if q_end is None:
+        q_end = 1 << N
+    states = torch.empty(S, dtype=torch.int64, device=J.device)
+    energies = torch.empty(S, dtype=torch.float64, device=J.device)
+    with torch.cuda.device(J.device):
+        rc = load().ising_lowest_alg1(J.data_ptr(), h.data_ptr(), N, int(S), int(q_begin), int(q_end), int(chunk_log2),
+                                      states.data_ptr(), energies.data_ptr(), _stream(stream))
+    _check(rc, "ising_lowest_alg1")
     return states, energies
 
 

@@ -295,6 +295,56 @@ int ising_lowest_host(const double* J_host, const double* h_host, int N, int S, 
     return ISING_OK;
 }
 
+int ising_lowest_alg1(const double* J_dev, const double* h_dev, int N, int S, uint64_t q_begin, uint64_t q_end,
+                      int chunk_log2, uint64_t* states_out_dev, double* energies_out_dev, void* stream)
+{
+    t_last_error.clear();
+    int rc = check_args(J_dev, h_dev, N, S, q_begin, q_end, states_out_dev, energies_out_dev);
+    if (rc != ISING_OK) return rc;
+    if (chunk_log2 < 10 || chunk_log2 > 20) { t_last_error = "chunk_log2 must be in [10, 20]"; return ISING_ERR_BAD_RANGE; }
+    rc = ensure_workspace();
+    if (rc != ISING_OK) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    Workspace& ws = t_ws;
+    ising_stats stats;
+    memset(&stats, 0, sizeof(stats));
+    CUDA_TRY(cudaEventRecord(ws.ev[0], st));
+    launch_stage(J_dev, h_dev, N, ws.tab, ws.ctrl, st, 0.0);          // validation only (same error codes)
+    stats.kernel_launches += 2;
+    CUDA_TRY(cudaMemcpyAsync(ws.h_ctrl, ws.ctrl, sizeof(Ctrl), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    if (ws.h_ctrl->status != ISING_OK && ws.h_ctrl->status != ISING_ERR_RANGE_W) {
+        t_last_error = std::string("instance rejected: ") + ising_strerror(ws.h_ctrl->status);
+        return ws.h_ctrl->status;
+    }
+    unsigned kept = 0;
+    const unsigned long long chunk = 1ull << chunk_log2;
+    for (unsigned long long cur = q_begin; cur < q_end; cur += chunk) {
+        const unsigned cnt = (unsigned)((q_end - cur) < chunk ? (q_end - cur) : chunk);
+        stats.kernel_launches += launch_alg1_chunk(J_dev, h_dev, N, cur, cnt, ws.pool, kept, st);
+        stats.enum_launches += 1;
+        stats.configs += cnt;
+        stats.candidates += cnt;
+        kept = kept + cnt < (unsigned)S ? kept + cnt : (unsigned)S;
+    }
+    stats.kernel_launches += launch_emit(ws.pool, S, (unsigned long long*)states_out_dev, energies_out_dev, st);
+    CUDA_TRY(cudaEventRecord(ws.ev[1], st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    CUDA_TRY(cudaGetLastError());
+    float total_ms = 0.f;
+    CUDA_TRY(cudaEventElapsedTime(&total_ms, ws.ev[0], ws.ev[1]));
+    stats.total_ms = total_ms;
+    stats.enum_ms = total_ms;
+    stats.exact = 1;
+    stats.keep = S;
+    stats.passes = 1;
+    stats.kernel_variant = 1;
+    stats.screen_shift = -1;
+    t_stats = stats;
+    t_have_stats = true;
+    return ISING_OK;
+}
+
 int ising_lowest_h0(const double* J_dev, int N, int S, uint64_t* states_out_dev, double* energies_out_dev, void* stream)
 {
     t_last_error.clear();

@@ -125,6 +125,9 @@ int  launch_merge_lists(const unsigned long long* states, const double* energies
                         unsigned long long* states_out, double* energies_out, cudaStream_t st);
 int  launch_expand_complements(const unsigned long long* states, const double* energies, int n, int N, int S,
                                Entry* scratch, unsigned long long* states_out, double* energies_out, cudaStream_t st);
+int  launch_alg1_chunk(const double* J, const double* h, int N, unsigned long long base, unsigned count,
+                       Entry* pool, unsigned kept, cudaStream_t st);
+int  launch_emit(const Entry* pool, int S, unsigned long long* states_out, double* energies_out, cudaStream_t st);
 // peak.cu
 double run_fma_peak(double ms_target, cudaStream_t st, int which);
 

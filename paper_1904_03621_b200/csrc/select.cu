@@ -258,6 +258,34 @@ __global__ void pack_kernel(const unsigned long long* __restrict__ states, const
     scratch[i] = e;
 }
 
+// ---- the paper's own pipeline (Algorithm 1), written plainly: for comparison on the same box ----
+// energies[j], states[j] of one chunk by direct evaluation of eq. (1) per state (O(N^2) each,
+// PAPER.md:170), appended behind the `kept` lowest found so far (the paper's low_en / low_st).
+__global__ void alg1_chunk_kernel(const double* __restrict__ J, const double* __restrict__ h, int N,
+                                  unsigned long long base, unsigned count, Entry* __restrict__ dst)
+{
+    const unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= count) return;
+    Entry e;
+    e.q = base + i;
+    e.key = key_from_f64(energy_f64(J, h, N, e.q, 0));
+    dst[i] = e;
+}
+
+// One iteration of Algorithm 1: evaluate the chunk, then select_lowest over (kept + chunk) by a full sort.
+int launch_alg1_chunk(const double* J, const double* h, int N, unsigned long long base, unsigned count,
+                      Entry* pool, unsigned kept, cudaStream_t st)
+{
+    alg1_chunk_kernel<<<(count + 127) / 128, 128, 0, st>>>(J, h, N, base, count, pool + kept);
+    return 1 + sort_pool(pool, kept + count, st);
+}
+
+int launch_emit(const Entry* pool, int S, unsigned long long* states_out, double* energies_out, cudaStream_t st)
+{
+    emit_kernel<<<(S + 255) / 256, 256, 0, st>>>(pool, S, states_out, energies_out);
+    return 1;
+}
+
 // h = 0: E(q) = E(~q). Every kept state of the lower half space brings its complement (same energy) with it.
 __global__ void expand_complement_kernel(const unsigned long long* __restrict__ states, const double* __restrict__ energies,
                                          int n, unsigned long long mask, Entry* __restrict__ scratch)

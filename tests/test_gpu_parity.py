@@ -480,3 +480,19 @@ def test_zero_field_symmetry_entry_point(B):
     qo, eo = load_golden(os.path.join(os.path.dirname(__file__), "golden", "cfg2.txt"))
     q1, e1 = B.ising_lowest_h0(c.J, c.S)
     assert_exact(B.states_to_numpy(q1), e1.cpu().numpy(), qo[:c.S], eo[:c.S])
+
+
+def test_paper_algorithm1_path(B):
+    """ising_lowest_alg1 (the paper's chunk / direct-energy / select pipeline) against the oracle and the main path."""
+    import torch
+    for (J, h), S, ch in ((I.complete_gaussian(18, seed=1818), 300, 12), (I.random_integer(21, seed=2121, wmax=2, density=0.3), 1000, 20),
+                          (I.complete_gaussian(11, seed=11), 1 << 11, 10)):
+        q, e = B.ising_lowest_alg1(J, h, S, chunk_log2=ch)
+        qo, eo = oracle.lowest(J, h, S)
+        assert_exact(B.states_to_numpy(q), e.cpu().numpy(), qo, eo)
+    c = I.baseline_config(5)
+    lo, hi = 77 << 24, 78 << 24
+    qa, ea = B.ising_lowest_alg1(c.J, c.h, c.S, lo, hi)
+    assert B.last_stats().kernel_variant == 1
+    qm, em = B.ising_lowest_range(c.J, c.h, c.S, lo, hi)
+    assert torch.equal(qa, qm) and torch.equal(ea, em)
