@@ -90,6 +90,7 @@ struct Piece {
     unsigned long long base;
     unsigned nthreads;
     int Lw;
+    bool direct;                    // the priming piece: one thread per state (direct_kernel)
 };
 
 // mode 0: (J, h) is an Ising instance, energies by eq. (1). mode 1: (Jorig, horig) = QUBO (a, b); (J, h) its Ising image.
@@ -102,6 +103,7 @@ int run_lowest(const double* J, const double* h, const double* Jorig, const doub
     memset(&stats, 0, sizeof(stats));
     const int lw_run = env_int("ISING_LW", LW_MAX, 0, LW_MAX);
     const int chunk_log2 = env_int("ISING_CHUNK_LOG2", 42, MIN_CHUNK_BITS, 44);
+    const int growth = env_int("ISING_GROWTH", 3, 1, 1 << 20);   // a launch is at most growth x what has been processed
     const int variant = env_int("ISING_KERNEL", 16, 16, 32) == 32 ? 32 : 16;   // 16: packed screen, 32: int32 kernel
 
     CUDA_TRY(cudaEventRecord(ws.ev[0], st));
@@ -124,7 +126,7 @@ int run_lowest(const double* J, const double* h, const double* Jorig, const doub
     double enum_ms = 0.0;
     unsigned kept = 0;
     if (N <= N_DIRECT_MAX) {
-        launch_direct(ws.tab, ws.ctrl, ws.pool, N, st);
+        launch_direct(ws.tab, ws.ctrl, ws.pool, N, 0, 1u << N, 0, st);
         stats.kernel_launches += 1;
         stats.enum_launches += 1;
         stats.configs = 1ull << N;
@@ -143,7 +145,7 @@ int run_lowest(const double* J, const double* h, const double* Jorig, const doub
                 const unsigned long long remaining = q_end - cur;
                 unsigned long long target = 1ull << MIN_CHUNK_BITS;
                 if (processed > 0) {
-                    target = 3 * processed;
+                    target = (unsigned long long)growth * processed;
                     if (target > (1ull << chunk_log2)) target = 1ull << chunk_log2;
                     if (!tau_finite && target > (1ull << 16)) target = 1ull << 16;   // everything passes: keep it small
                 }
@@ -159,10 +161,13 @@ int run_lowest(const double* J, const double* h, const double* Jorig, const doub
                 pc.base = cur;
                 pc.nthreads = (unsigned)nt;
                 pc.Lw = Lw;
+                pc.direct = (processed == 0);          // a2': the first 2^15 states, tau = +inf
                 cur += nt << (LOWBITS + Lw);
             }
             CUDA_TRY(cudaEventRecord(ws.ev[2], st));
-            if (variant == 16) launch_enumerate16(ws.tab, ws.ctrl, ws.pool, N, pc.Lw, pc.base, pc.nthreads, st);
+            if (pc.direct) launch_direct(ws.tab, ws.ctrl, ws.pool, N, pc.base, pc.nthreads << (LOWBITS + pc.Lw), 0, st);
+            else if (variant == 16) launch_enumerate16(ws.tab, ws.ctrl, ws.pool, N, pc.Lw, pc.base, pc.nthreads,
+                                                       processed < (1ull << 30), st);
             else launch_enumerate(ws.tab, ws.ctrl, ws.pool, N, pc.Lw, pc.base, pc.nthreads, st);
             CUDA_TRY(cudaEventRecord(ws.ev[3], st));
             stats.kernel_launches += 1;
@@ -181,6 +186,7 @@ int run_lowest(const double* J, const double* h, const double* Jorig, const doub
                 stats.kernel_launches += 1;
                 stats.split_retries += 1;
                 Piece a = pc, b = pc;
+                a.direct = b.direct = false;
                 if (pc.nthreads >= 64) {
                     a.nthreads = pc.nthreads / 64 * 32;
                     b.nthreads = pc.nthreads - a.nthreads;

@@ -111,10 +111,11 @@ void launch_qubo_to_ising(const double* a, const double* b, int N, double* J, do
 // enumerate.cu
 void launch_enumerate(const Tables* tab, Ctrl* ctrl, Entry* pool, int N, int Lw,
                       unsigned long long base, unsigned nthreads, cudaStream_t st);
-void launch_direct(const Tables* tab, Ctrl* ctrl, Entry* pool, int N, cudaStream_t st);
+void launch_direct(const Tables* tab, Ctrl* ctrl, Entry* pool, int N, unsigned long long base, unsigned count,
+                   unsigned kept, cudaStream_t st);
 // enumerate16.cu
 void launch_enumerate16(const Tables* tab, Ctrl* ctrl, Entry* pool, int N, int Lw,
-                        unsigned long long base, unsigned nthreads, cudaStream_t st);
+                        unsigned long long base, unsigned nthreads, bool heavy_hits, cudaStream_t st);
 // select.cu
 int  launch_select(Entry* pool, Ctrl* ctrl, unsigned n, int S, cudaStream_t st);     // returns kernels launched
 int  launch_final(const double* J, const double* h, int N, int mode, Entry* pool, unsigned m, int S,

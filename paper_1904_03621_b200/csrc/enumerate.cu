@@ -173,17 +173,21 @@ enumerate_kernel(const Tables* __restrict__ tab, Ctrl* __restrict__ ctrl, Entry*
     }
 }
 
-// N <= N_DIRECT_MAX (2^N <= 16384 states): every state's grid energy by eq. (1) directly; all go to the pool.
-__global__ void direct_kernel(const Tables* __restrict__ tab, Ctrl* __restrict__ ctrl, Entry* __restrict__ pool, int N)
+// Direct evaluation of eq. (1) on the grid for `count` consecutive states starting at `base`; every state goes to the
+// pool behind the `kept` entries already there. Used for the whole space when N <= N_DIRECT_MAX (2^N <= 16384 states)
+// and for the first 2^15 states of any larger run (a2': with tau = +inf everything passes anyway, and one thread per
+// state is the fastest way to form them).
+__global__ void direct_kernel(const Tables* __restrict__ tab, Ctrl* __restrict__ ctrl, Entry* __restrict__ pool, int N,
+                              unsigned long long base, unsigned count, unsigned kept)
 {
-    const unsigned total = 1u << N;
-    for (unsigned q = blockIdx.x * blockDim.x + threadIdx.x; q < total; q += gridDim.x * blockDim.x) {
+    for (unsigned t = blockIdx.x * blockDim.x + threadIdx.x; t < count; t += gridDim.x * blockDim.x) {
+        const unsigned long long q = base + t;
         int e = 0;
         for (int i = 0; i < N; ++i) {
-            const unsigned bi = (q >> i) & 1u;
+            const unsigned bi = (unsigned)(q >> i) & 1u;
             for (int j = i + 1; j < N; ++j) {
                 const int v = tab->Jq[i * 64 + j];
-                e += (bi ^ ((q >> j) & 1u)) ? v : -v;
+                e += (bi ^ ((unsigned)(q >> j) & 1u)) ? v : -v;
             }
             const int hv = tab->hq[i];
             e += bi ? -hv : hv;
@@ -191,9 +195,9 @@ __global__ void direct_kernel(const Tables* __restrict__ tab, Ctrl* __restrict__
         Entry en;
         en.key = key_from_i32(e);
         en.q = q;
-        pool[q] = en;
+        pool[kept + t] = en;
     }
-    if (blockIdx.x == 0 && threadIdx.x == 0) ctrl->count = total;
+    if (blockIdx.x == 0 && threadIdx.x == 0) ctrl->count = kept + count;
 }
 
 void launch_enumerate(const Tables* tab, Ctrl* ctrl, Entry* pool, int N, int Lw,
@@ -204,11 +208,11 @@ void launch_enumerate(const Tables* tab, Ctrl* ctrl, Entry* pool, int N, int Lw,
     enumerate_kernel<<<blocks, threads, 0, st>>>(tab, ctrl, pool, N, Lw, base, nthreads);
 }
 
-void launch_direct(const Tables* tab, Ctrl* ctrl, Entry* pool, int N, cudaStream_t st)
+void launch_direct(const Tables* tab, Ctrl* ctrl, Entry* pool, int N, unsigned long long base, unsigned count,
+                   unsigned kept, cudaStream_t st)
 {
-    const unsigned total = 1u << N;
-    const unsigned threads = 256, blocks = (total + threads - 1) / threads;
-    direct_kernel<<<blocks, threads, 0, st>>>(tab, ctrl, pool, N);
+    const unsigned threads = 128, blocks = (count + threads - 1) / threads;
+    direct_kernel<<<blocks, threads, 0, st>>>(tab, ctrl, pool, N, base, count, kept);
 }
 
 }  // namespace ising
