@@ -5,17 +5,20 @@
 // fixed point: one unit = 2^s grid units, every table entry rounded DOWN, so that
 //      V16[lo] + C16[mid][lo] + U16[mid]  <=  (V[lo] + C[mid][lo] + U[mid]) / 2^s            (a rigorous lower bound)
 // and the inner operation  m = min(V16 + C16, m)  is one VIADDMNMX.U16x2 for the two configurations (lo, mid) and
-// (lo, mid + 16): 512 + 16 ALU instructions per 1024 configurations instead of 1024 + 32. A block whose bound is
+// (lo, mid | 8): 512 + 16 ALU instructions per 1024 configurations instead of 1024 + 32. A block whose bound is
 // <= tau is formed again by the whole warp in exact int32 grid arithmetic (the same a4 path as enumerate.cu), so
 // what reaches the pool -- and everything after it -- is identical to the int32 kernel; the 16-bit screen can only
 // cause extra (false) hits, never a miss. For integer instances with small weights s = 0 and the screen is exact.
 //
-// Representation (so that no 16-bit lane ever wraps, stage.cu chooses s accordingly):
-//   Vp[lo]  both halves = V16[lo] + 32768                       (biased, in [0, 65535])
-//   Cp[r][lo] = ( C16[r][lo] , C16[r+16][lo] )                  (two's complement halves; the lane add is mod 2^16)
-//   Up[r]   = ( U16[r] + cU , U16[r+16] + cU )                  (offset cU >= |U16|: non-negative halves)
+// Representation (so that no 16-bit lane ever wraps, stage.cu chooses s accordingly); m0(u) = (u & 7) | ((u >> 3) << 4):
+//   Va[lo]  both halves = V16[lo] + 32768                       (biased, in [0, 65535]); mid bit 4 clear
+//   Vb[lo]  both halves = floor((V[lo] + C[16][lo]) / 2^s) + 32768                       mid bit 4 set
+//   Cp[u][lo] = ( C16[m0(u)][lo] , C16[m0(u) | 8][lo] )         (two's complement halves; the lane add is mod 2^16)
+//   Up[u]   = ( U16[m0(u)] + cU , U16[m0(u) | 8] + cU )         (offset cU >= |U16|: non-negative halves)
 //   block bound = min over halves of g  -  32768 - cU
-// Because every half of Vp and Up is a non-negative number that stays inside its 16 bits, a Gray step may update
+// The two halves of a word differ in mid bit 3; mid bit 4 is resolved by the two register sets Va / Vb, which both
+// consume the SAME row of Cp (rows u < 8 only): one warp-uniform LDS.128 feeds 8 add-mins.
+// Because every half of Va, Vb and Up is a non-negative number that stays inside its 16 bits, a Gray step may update
 // the packed words with plain 32-bit integer adds of the packed delta (d_lo + 65536 d_hi): those run as IMAD on the
 // FMA pipe, off the ALU pipe that bounds the kernel.
 //
@@ -25,6 +28,11 @@
 //
 // Base state (a2): the block computes the local fields Phi_i and the energy of its base state (thread bits zero)
 // once in shared memory; a thread adds the contribution of its own <= 8 thread bits, O(8 N_low) instead of O(N^2).
+//
+// Register allocation matters: every VIADDMNMX reads three distinct registers, and ptxas's choice of even/odd
+// register banks for them decides whether the instruction takes 2 or 3 register-file cycles. The statement order
+// of the inline hit path below is the one for which ptxas 12.9 finds a conflict-free allocation (6 of 528 add-mins
+// with three same-bank sources instead of 128; 2.5 % in throughput) -- check with cuobjdump after touching it.
 #include "common.cuh"
 
 namespace ising {
