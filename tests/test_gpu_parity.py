@@ -198,6 +198,39 @@ def _neighbour_check(J, h, q, e, nflip=2, seeds=None):
         assert (float(ee), int(x)) > last, f"missed neighbour {int(x)} with energy {ee}"
 
 
+def _descent_check(J, h, q, e, restarts, seed):
+    """Independent search from the other side: greedy single-flip descents from random states (numpy, vectorised).
+    Every local minimum they reach, and every state on the way, that lies below the returned S-th entry must be in
+    the returned list. Energies are taken from the oracle's single-state function."""
+    N = len(h)
+    rng = np.random.default_rng(seed)
+    s = 2.0 * rng.integers(0, 2, size=(restarts, N)) - 1.0
+    seen = set()
+    for _ in range(4 * N):
+        phi = s @ J + h                                   # local fields; flipping i changes E by 2 s_i phi_i
+        gain = 2.0 * s * phi
+        i = np.argmin(gain, axis=1)
+        g = gain[np.arange(restarts), i]
+        move = g < 0
+        if not move.any():
+            break
+        s[move, i[move]] *= -1.0
+    bits = (s > 0).astype(np.uint64)
+    states = (bits << np.arange(N, dtype=np.uint64)[None, :]).sum(axis=1).astype(np.uint64)
+    states = np.unique(states)
+    en = oracle.energies_of(J, h, states)
+    have = set(int(x) for x in q)
+    last = (float(e[-1]), int(q[-1]))
+    found_in_list = 0
+    for x, ee in zip(states, en):
+        if int(x) in have:
+            found_in_list += 1
+        else:
+            assert (float(ee), int(x)) > last, f"descent found state {int(x)} with energy {ee} below the S-th entry"
+    assert found_in_list >= 1, "the descents never reached any returned state: the check has no power"
+    return found_in_list
+
+
 def test_config4_full_run_properties(B):
     c = I.baseline_config(4)
     q, e = gpu_lowest(B, c.J, c.h, c.S)
@@ -419,6 +452,11 @@ def test_config5_full_run_properties(B):
     pairs = list(zip(e.tolist(), q.tolist()))
     assert pairs == sorted(pairs) and len(set(q.tolist())) == c.S
     _neighbour_check(c.J, c.h, q, e, nflip=2)
+    _descent_check(c.J, c.h, q, e, restarts=60000, seed=55)
+    # the int32 kernel (one add-min per configuration, no 16-bit screen) must return the same list on the full space
+    q32, e32 = _with_kernel(32, lambda: gpu_lowest(B, c.J, c.h, c.S))
+    assert B.last_stats().kernel_variant == 32
+    assert q32.tolist() == q.tolist() and e32.tolist() == e.tolist()
     rng = np.random.default_rng(5)
     g = 2.0 * rng.integers(0, 2, size=c.N) - 1.0
     mask = np.uint64(sum(1 << i for i in range(c.N) if g[i] < 0))
