@@ -534,3 +534,34 @@ def test_paper_algorithm1_path(B):
     assert B.last_stats().kernel_variant == 1
     qm, em = B.ising_lowest_range(c.J, c.h, c.S, lo, hi)
     assert torch.equal(qa, qm) and torch.equal(ea, em)
+
+
+def test_concurrent_host_threads_and_streams(B):
+    """include/ising.h: workspaces are per host thread, calls on different streams may run concurrently."""
+    import threading
+    import torch
+    insts = [I.complete_gaussian(24, seed=240 + t) for t in range(4)]
+    want = [oracle.lowest(J, h, 64) for J, h in insts]
+    got = [None] * 4
+    errs = []
+
+    def work(t):
+        try:
+            torch.cuda.set_device(0)
+            st = torch.cuda.Stream()
+            with torch.cuda.stream(st):
+                for _ in range(3):
+                    q, e = B.ising_lowest(insts[t][0], insts[t][1], 64, stream=st)
+                st.synchronize()
+            got[t] = (B.states_to_numpy(q), e.cpu().numpy())
+        except Exception as ex:            # noqa: BLE001
+            errs.append(repr(ex))
+
+    threads = [threading.Thread(target=work, args=(t,)) for t in range(4)]
+    for th in threads:
+        th.start()
+    for th in threads:
+        th.join()
+    assert not errs, errs
+    for t in range(4):
+        assert_exact(got[t][0], got[t][1], want[t][0], want[t][1])
