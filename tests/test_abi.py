@@ -67,6 +67,11 @@ def test_argument_validation_precedes_cuda(lib):
     assert lib.ising_merge_lists(qp, ep, 4, 5, qp, ep, None) == B.ERR_BAD_S
     assert lib.ising_energies(Jp, hp, 20, None, 4, ep, None) == B.ERR_NULL
     assert lib.ising_get_last_stats(None) == B.ERR_NULL
+    assert lib.ising_lowest_h0(None, 20, 16, qp, ep, None) == B.ERR_NULL
+    assert lib.ising_lowest_h0(Jp, 0, 16, qp, ep, None) == B.ERR_BAD_N
+    assert lib.ising_lowest_alg1(Jp, hp, 20, 16, 0, 1 << 20, 25, qp, ep, None) == B.ERR_BAD_RANGE   # chunk_log2 > 20
+    assert lib.ising_lowest_alg1(Jp, None, 20, 16, 0, 1 << 20, 20, qp, ep, None) == B.ERR_NULL
+    assert lib.ising_addmin16x2_peak(1.0, None, None) == B.ERR_NULL
     assert lib.ising_fma_peak(1.0, None, None) == B.ERR_NULL
     # N = 24: ranges must be multiples of 2^20
     J = np.zeros((24, 24)); h = np.zeros(24)
