@@ -47,6 +47,10 @@ def parse_args():
     ap.add_argument("--config", type=int, default=5, help="BASELINE.json config number (1-based); 5 = N=48")
     ap.add_argument("--range-log2", type=int, default=0,
                     help="development only: enumerate just the first 2^r states per step (0 = the whole space)")
+    ap.add_argument("--sharded", action="store_true",
+                    help="N > 1: ONE instance, its state space cut into one aligned range per rank, lists exchanged with "
+                         "an all-gather and merged (paper_1904_03621_b200/sharded.py): strong scaling. Default: every "
+                         "rank enumerates its own instance (weak scaling, no data-path collective)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -201,7 +205,8 @@ def main():
         dist.barrier()
     B.load()
 
-    inst = instance_for_rank(args.config, rank)
+    sharded_mode = args.sharded and world > 1
+    inst = instance_for_rank(args.config, 0 if sharded_mode else rank)
     N, S = inst.N, inst.S
     q_end = 1 << N
     if args.range_log2:
@@ -214,7 +219,11 @@ def main():
     stream = torch.cuda.current_stream()
 
     def step():
-        B.ising_lowest_range(J, h, S, 0, q_end, stream=stream, out=out)
+        if sharded_mode:
+            from paper_1904_03621_b200 import sharded
+            sharded.ising_lowest_sharded(J, h, S)          # every rank ends with the global list
+        else:
+            B.ising_lowest_range(J, h, S, 0, q_end, stream=stream, out=out)
         return B.last_stats()
 
     def barrier():
@@ -240,6 +249,7 @@ def main():
     enum_ms = 0.0
     enum_launches = 0
     launches = 0
+    enum_configs = 0
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     for _ in range(args.steps):
         flush.zero_()                       # L2 flush between timed iterations (outside the event bracket)
@@ -249,6 +259,7 @@ def main():
         ev1.synchronize()
         dev_ms += ev0.elapsed_time(ev1)
         enum_ms += st.enum_ms
+        enum_configs += st.configs
         enum_launches += st.enum_launches
         launches += st.kernel_launches
     barrier()
@@ -257,7 +268,7 @@ def main():
 
     # ---- end to end: pinned host buffers in, host buffers out, through ising_lowest_host ----
     e2e = None
-    if not args.no_e2e:
+    if not args.no_e2e and not sharded_mode:
         Jh = torch.from_numpy(inst.J).pin_memory()
         hh = torch.from_numpy(inst.h).pin_memory()
         qh = torch.empty(S, dtype=torch.int64).pin_memory()
@@ -278,7 +289,7 @@ def main():
     if world > 1:
         dist.all_reduce(times, op=dist.ReduceOp.MAX)
     dev_ms_max, e2e_s_max = float(times[0]), float(times[1])
-    total_configs = float(configs_per_step) * args.steps * world
+    total_configs = float(configs_per_step) * args.steps * (1 if sharded_mode else world)
     value = total_configs / (dev_ms_max * 1e-3)
 
     if rank == 0:
@@ -294,7 +305,7 @@ def main():
         live_peak = addmin16x2_peak * 2 if st.kernel_variant == 16 else addmin_peak
         kname = "ising::enumerate16_kernel" if st.kernel_variant == 16 else "ising::enumerate_kernel"
         fma_nominal = sms * FMA_LANES_PER_CLK_PER_SM * sm_max_hz       # FMA / s
-        achieved = float(configs_per_step) * args.steps / (enum_ms * 1e-3)   # one add-min per configuration
+        achieved = float(enum_configs) / (enum_ms * 1e-3)   # this rank's kernel: one add-min per configuration
         traffic = None
         tpath = os.path.join(ROOT, "profiles", "enumerate_dram_bytes_per_launch.txt")
         if os.path.exists(tpath):
@@ -305,12 +316,13 @@ def main():
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": dev_ms_max / args.steps, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None,
+            "scaling": "strong" if sharded_mode else "weak", "vs_baseline": None,
             "dtype": "int16x2 screen + int32 exact (fp64 output)" if st.kernel_variant == 16 else "int32 (fp64 output)",
             "data": "synthetic",
             "config": {"workload": f"BASELINE.json configs[{args.config - 1}]: {inst.name}, N={N}, S={S}, "
                                    f"states [0, 2^{q_end.bit_length() - 1}) of 2^{N} per step",
-                       "parallelism": f"independent instances x{world}" if world > 1 else "single GPU",
+                       "parallelism": (f"one instance, {world} state ranges + all-gather + merge" if sharded_mode else
+                                       f"independent instances x{world}" if world > 1 else "single GPU"),
                        "l2": "256 MiB buffer written between timed steps (inputs are 18 KB; the path has no HBM traffic)",
                        "grid_exponent_p": st.grid_exponent, "epsilon": st.epsilon, "kept": st.keep,
                        "kernel_variant": st.kernel_variant, "screen_shift": st.screen_shift,
