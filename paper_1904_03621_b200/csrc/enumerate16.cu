@@ -115,7 +115,7 @@ __global__ void __launch_bounds__(E16_THREADS, 2)
 enumerate16_kernel(const Tables* __restrict__ tab, Ctrl* __restrict__ ctrl, Entry* __restrict__ pool,
                    int N, int Lw, unsigned long long base, unsigned nthreads)
 {
-    __shared__ __align__(16) unsigned sCp[NHALF * NLO];
+    __shared__ __align__(16) unsigned sCp[(NHALF / 2) * NLO];   // rows u < 8 (mid bit 4 clear); set b covers the rest
     __shared__ __align__(16) unsigned sDVp[LW_MAX * 2 * NLO];
     __shared__ __align__(16) unsigned sDUp[LW_MAX * 2 * NHALF];
     __shared__ int sC[NMID * NLO];
@@ -129,7 +129,7 @@ enumerate16_kernel(const Tables* __restrict__ tab, Ctrl* __restrict__ ctrl, Entr
     const int nlow = LOWBITS + Lw;
     const unsigned long long qB = base + ((unsigned long long)(blockIdx.x * blockDim.x) << nlow);
 
-    for (int i = threadIdx.x; i < NHALF * NLO; i += blockDim.x) sCp[i] = tab->Cp[i];
+    for (int i = threadIdx.x; i < (NHALF / 2) * NLO; i += blockDim.x) sCp[i] = tab->Cp[i];
     for (int i = threadIdx.x; i < LW_MAX * 2 * NLO; i += blockDim.x) sDVp[i] = tab->DVp[i];
     for (int i = threadIdx.x; i < LW_MAX * 2 * NHALF; i += blockDim.x) sDUp[i] = tab->DUp[i];
     for (int i = threadIdx.x; i < NMID * NLO; i += blockDim.x) sC[i] = tab->C[i];
