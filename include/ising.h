@@ -96,6 +96,20 @@ int ising_merge_lists(const uint64_t *states_in_dev, const double *energies_in_d
                       uint64_t *states_out_dev, double *energies_out_dev, void *stream);
 
 /*
+ * ising_dos -- density of states (cf. the paper's Fig. 6): the histogram
+ * of ALL 2^N energies of eq. (1). Every energy is formed exactly on the library's 2^-p grid (the instance rounded to
+ * multiples of 2^-p; for integer / dyadic instances that is the instance itself, otherwise each energy is within
+ * ising_stats.epsilon of eq. (1)) and counted:
+ *      hist_out_dev[b] = #{ q : e_lo + b * width <= E_grid(q) < e_lo + (b + 1) * width },   0 <= b < nbins
+ * with e_lo = -(sum of |grid weights|) and width the smallest power-of-two multiple of 2^-p for which nbins bins
+ * cover [-sum, +sum]; both are written to the two host doubles. 2 <= nbins <= 4096. sum_b hist[b] = 2^N.
+ * J_dev, h_dev as in ising_lowest; hist_out_dev [nbins] uint64 device memory. Bound by shared-memory atomics
+ * (about 10^12 states/s), not the hot path.
+ */
+int ising_dos(const double *J_dev, const double *h_dev, int N, int nbins, uint64_t *hist_out_dev,
+              double *e_lo_out_host, double *bin_width_out_host, void *stream);
+
+/*
  * ising_lowest_alg1 -- the PAPER'S OWN pipeline (Algorithm 1), written plainly for this GPU, as the
  * on-box comparison for the design above: the range is cut into chunks of
  * 2^chunk_log2 states (10 <= chunk_log2 <= 20); every state's energy is evaluated directly by eq. (1) in fp64,
@@ -151,7 +165,7 @@ typedef struct ising_stats {
     double   total_ms;           /* device time of the whole call */
     int32_t  keep;               /* K: candidates kept per list */
     int32_t  inner_bits;         /* L: unrolled Gray bits per inner block */
-    int32_t  kernel_variant;     /* 1: ising_lowest_alg1. 16: packed 16-bit screen + exact int32 re-forming of hit blocks (default);
+    int32_t  kernel_variant;     /* 1: ising_lowest_alg1. 2: ising_dos. 16: packed 16-bit screen + exact int32 re-forming of hit blocks (default);
                                     32: int32 add-min per configuration (environment ISING_KERNEL=32) */
     int32_t  screen_shift;       /* variant 16: one 16-bit unit = 2^screen_shift grid units (0: screen is exact) */
 } ising_stats;

@@ -173,6 +173,38 @@ int64_t oracle_lowest(const double *J, const double *h, int N, int64_t S,
     return n_out;
 }
 
+/*
+ * Density of states (cf. the paper's Fig. 6): hist[b] = number of states q in [0, 2^N) with
+ * e_lo + b*width <= E(q) < e_lo + (b+1)*width, E by eq. (1) as above. Returns the number of states that fell
+ * outside [e_lo, e_lo + nbins*width) (they are not counted), or -1 on bad arguments.
+ * Pins (tests/test_oracle_pins.py): binomial level counts of the uniform ferromagnet and of a uniform field.
+ */
+int64_t oracle_dos(const double *J, const double *h, int N, double e_lo, double width, int nbins, uint64_t *hist)
+{
+    if (!J || !h || !hist || N < 1 || N > 40 || nbins < 1 || !(width > 0.0)) return -1;
+    for (int b = 0; b < nbins; ++b) hist[b] = 0;
+    const int64_t total = (int64_t)1 << N;
+    int64_t outside = 0;
+#pragma omp parallel
+    {
+        uint64_t *loc = (uint64_t *)calloc((size_t)nbins, sizeof(uint64_t));
+        int64_t out_loc = 0;
+#pragma omp for schedule(static)
+        for (int64_t q = 0; q < total; ++q) {
+            const double b = floor((oracle_energy(J, h, N, (uint64_t)q) - e_lo) / width);
+            if (b < 0.0 || b >= (double)nbins) ++out_loc;
+            else ++loc[(int)b];
+        }
+#pragma omp critical
+        {
+            for (int b = 0; b < nbins; ++b) hist[b] += loc[b];
+            outside += out_loc;
+        }
+        free(loc);
+    }
+    return outside;
+}
+
 int oracle_max_threads(void)
 {
 #ifdef _OPENMP

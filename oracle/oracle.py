@@ -43,6 +43,8 @@ def _load():
         lib.oracle_lowest.argtypes = [dp, dp, ctypes.c_int, ctypes.c_int64, ctypes.c_uint64,
                                       ctypes.c_uint64, up, dp, ctypes.c_int]
         lib.oracle_max_threads.restype = ctypes.c_int
+        lib.oracle_dos.restype = ctypes.c_int64
+        lib.oracle_dos.argtypes = [dp, dp, ctypes.c_int, ctypes.c_double, ctypes.c_double, ctypes.c_int, up]
         _lib = lib
     return _lib
 
@@ -92,6 +94,17 @@ def lowest(J, h, S: int, q_begin: int = 0, q_end: int | None = None, threads: in
     if n < 0:
         raise ValueError("oracle_lowest: bad arguments")
     return states[:n].copy(), en[:n].copy()
+
+
+def dos(J, h, e_lo: float, width: float, nbins: int):
+    """Histogram of all 2^N energies of eq. (1): (hist uint64[nbins], number of states outside the bins)."""
+    J, h, N, Jp, hp = _prep(J, h)
+    hist = np.zeros(nbins, dtype=np.uint64)
+    out = _load().oracle_dos(Jp, hp, N, float(e_lo), float(width), int(nbins),
+                             hist.ctypes.data_as(ctypes.POINTER(ctypes.c_uint64)))
+    if out < 0:
+        raise ValueError("oracle_dos: bad arguments")
+    return hist, int(out)
 
 
 _SO_GRAY = os.path.join(_HERE, "liboracle_gray.so")

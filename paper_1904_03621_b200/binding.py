@@ -20,7 +20,7 @@ N_MAX = 63
 S_MAX = 65536
 
 # every symbol include/ising.h declares (tests/test_abi.py checks the header against this list and the .so)
-EXPORTS = ["ising_lowest", "ising_lowest_range", "ising_lowest_host", "ising_lowest_h0", "ising_lowest_alg1", "ising_merge_lists", "qubo_lowest",
+EXPORTS = ["ising_lowest", "ising_lowest_range", "ising_lowest_host", "ising_lowest_h0", "ising_lowest_alg1", "ising_dos", "ising_merge_lists", "qubo_lowest",
            "ising_energies", "ising_get_last_stats", "ising_strerror", "ising_last_error", "ising_version",
            "ising_fma_peak", "ising_addmin_peak", "ising_addmin16x2_peak", "ising_release_workspace"]
 
@@ -85,6 +85,8 @@ def load():
     lib.ising_lowest_h0.argtypes = [dp, i32, i32, up, dp, vp]
     lib.ising_lowest_alg1.argtypes = [dp, dp, i32, i32, u64, u64, i32, up, dp, vp]
     lib.ising_lowest_alg1.restype = ctypes.c_int
+    lib.ising_dos.argtypes = [dp, dp, i32, i32, up, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double), vp]
+    lib.ising_dos.restype = ctypes.c_int
     lib.ising_lowest_h0.restype = ctypes.c_int
     lib.qubo_lowest.argtypes = [dp, dp, i32, i32, up, dp, vp]
     lib.ising_energies.argtypes = [dp, dp, i32, up, i64, dp, vp]
@@ -195,6 +197,21 @@ def ising_lowest_alg1(J, h, S: int, q_begin: int = 0, q_end: int | None = None, 
                                       states.data_ptr(), energies.data_ptr(), _stream(stream))
     _check(rc, "ising_lowest_alg1")
     return states, energies
+
+
+def ising_dos(J, h, nbins: int = 1024, stream=None):
+    """Density of states (include/ising.h): returns (hist int64 [nbins] device tensor, e_lo, bin_width)."""
+    import torch
+    h = _dev_f64(h, (len(h),))
+    N = h.shape[0]
+    J = _dev_f64(J, (N, N))
+    hist = torch.empty(nbins, dtype=torch.int64, device=J.device)
+    e_lo, width = ctypes.c_double(0.0), ctypes.c_double(0.0)
+    with torch.cuda.device(J.device):
+        rc = load().ising_dos(J.data_ptr(), h.data_ptr(), N, int(nbins), hist.data_ptr(), ctypes.byref(e_lo),
+                              ctypes.byref(width), _stream(stream))
+    _check(rc, "ising_dos")
+    return hist, e_lo.value, width.value
 
 
 def ising_lowest_h0(J, S: int, stream=None):

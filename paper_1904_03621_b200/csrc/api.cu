@@ -1,6 +1,7 @@
 // api.cu -- the C ABI of include/ising.h and the host driver that sequences the kernels.
 // No torch types, no exceptions across the boundary, no CPU fallback: without a CUDA device every compute entry
 // point returns ISING_ERR_CUDA.
+#include <cmath>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
@@ -298,6 +299,77 @@ int ising_lowest_host(const double* J_host, const double* h_host, int N, int S, 
     CUDA_TRY(cudaMemcpyAsync(states_out_host, ws.out_q, sizeof(uint64_t) * S, cudaMemcpyDeviceToHost, st));
     CUDA_TRY(cudaMemcpyAsync(energies_out_host, ws.out_e, sizeof(double) * S, cudaMemcpyDeviceToHost, st));
     CUDA_TRY(cudaStreamSynchronize(st));
+    return ISING_OK;
+}
+
+int ising_dos(const double* J_dev, const double* h_dev, int N, int nbins, uint64_t* hist_out_dev,
+              double* e_lo_out_host, double* bin_width_out_host, void* stream)
+{
+    t_last_error.clear();
+    if (!J_dev || !h_dev || !hist_out_dev || !e_lo_out_host || !bin_width_out_host) {
+        t_last_error = "null pointer argument";
+        return ISING_ERR_NULL;
+    }
+    if (N < 1 || N > ISING_N_MAX) { t_last_error = "N out of range"; return ISING_ERR_BAD_N; }
+    if (nbins < 2 || nbins > 4096) { t_last_error = "nbins must be in [2, 4096]"; return ISING_ERR_BAD_S; }
+    int rc = ensure_workspace();
+    if (rc != ISING_OK) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    Workspace& ws = t_ws;
+    ising_stats stats;
+    memset(&stats, 0, sizeof(stats));
+    CUDA_TRY(cudaEventRecord(ws.ev[0], st));
+    launch_stage(J_dev, h_dev, N, ws.tab, ws.ctrl, st, 0.0);
+    stats.kernel_launches += 2;
+    CUDA_TRY(cudaMemcpyAsync(ws.h_ctrl, ws.ctrl, sizeof(Ctrl), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    if (ws.h_ctrl->status != ISING_OK) {
+        t_last_error = std::string("instance rejected: ") + ising_strerror(ws.h_ctrl->status);
+        return ws.h_ctrl->status;
+    }
+    const int p = ws.h_ctrl->p;
+    // every grid energy lies in [-Wq, Wq], Wq = sum of the rounded |weights| <= W 2^p + (number of weights)
+    const long long Wq = (long long)ceil(ldexp(ws.h_ctrl->W, p)) + (long long)N * (N - 1) / 2 + N + 1;
+    const long long e_lo = -Wq;
+    int bshift = 0;
+    while (((2 * Wq) >> bshift) + 1 > (long long)nbins) ++bshift;
+    CUDA_TRY(cudaMemsetAsync(hist_out_dev, 0, sizeof(uint64_t) * (size_t)nbins, st));
+    if (N <= N_DIRECT_MAX) {
+        launch_dos_direct(ws.tab, N, (int)e_lo, bshift, (unsigned long long*)hist_out_dev, st);
+        stats.kernel_launches += 1;
+        stats.enum_launches += 1;
+    } else {
+        int Lw = N - LOWBITS - 12;
+        Lw = Lw < 0 ? 0 : (Lw > LW_MAX ? LW_MAX : Lw);
+        const unsigned long long total_threads = 1ull << (N - LOWBITS - Lw);       // >= 32 because N >= 15
+        const unsigned long long per_launch = 1ull << 22;
+        for (unsigned long long t0 = 0; t0 < total_threads; t0 += per_launch) {
+            const unsigned nt = (unsigned)((total_threads - t0) < per_launch ? (total_threads - t0) : per_launch);
+            launch_dos(ws.tab, N, Lw, t0 << (LOWBITS + Lw), nt, (int)e_lo, bshift, nbins,
+                       (unsigned long long*)hist_out_dev, st);
+            stats.kernel_launches += 1;
+            stats.enum_launches += 1;
+        }
+    }
+    CUDA_TRY(cudaEventRecord(ws.ev[1], st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    CUDA_TRY(cudaGetLastError());
+    float total_ms = 0.f;
+    CUDA_TRY(cudaEventElapsedTime(&total_ms, ws.ev[0], ws.ev[1]));
+    *e_lo_out_host = ldexp((double)e_lo, -p);
+    *bin_width_out_host = ldexp(1.0, bshift - p);
+    stats.configs = 1ull << N;
+    stats.grid_exponent = p;
+    stats.exact = ws.h_ctrl->exact;
+    stats.epsilon = ws.h_ctrl->epsilon;
+    stats.total_ms = total_ms;
+    stats.enum_ms = total_ms;
+    stats.passes = 1;
+    stats.kernel_variant = 2;
+    stats.screen_shift = -1;
+    stats.inner_bits = LOWBITS;
+    t_stats = stats;
+    t_have_stats = true;
     return ISING_OK;
 }
 

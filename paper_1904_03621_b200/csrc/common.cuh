@@ -129,6 +129,10 @@ int  launch_expand_complements(const unsigned long long* states, const double* e
 int  launch_alg1_chunk(const double* J, const double* h, int N, unsigned long long base, unsigned count,
                        Entry* pool, unsigned kept, cudaStream_t st);
 int  launch_emit(const Entry* pool, int S, unsigned long long* states_out, double* energies_out, cudaStream_t st);
+// dos.cu
+void launch_dos(const Tables* tab, int N, int Lw, unsigned long long base, unsigned nthreads, int e_lo, int bshift,
+                int nbins, unsigned long long* hist, cudaStream_t st);
+void launch_dos_direct(const Tables* tab, int N, int e_lo, int bshift, unsigned long long* hist, cudaStream_t st);
 // peak.cu
 double run_fma_peak(double ms_target, cudaStream_t st, int which);
 

@@ -565,3 +565,54 @@ def test_concurrent_host_threads_and_streams(B):
     assert not errs, errs
     for t in range(4):
         assert_exact(got[t][0], got[t][1], want[t][0], want[t][1])
+
+
+# ---------- density-of-states mode (ising_dos) ----------
+@pytest.mark.parametrize("N,kind", [(10, "int"), (14, "int"), (15, "int"), (18, "int"), (22, "int"), (12, "real"), (20, "real")])
+def test_dos_matches_oracle(B, N, kind):
+    """Integer instances: the grid is the instance, the histogram must equal the oracle's bin for bin.
+    Real instances: a state can change bins only if its energy is within epsilon of a bin edge."""
+    if kind == "int":
+        J, h = I.random_integer(N, seed=600 + N, wmax=3, density=0.5)
+    else:
+        J, h = I.complete_gaussian(N, seed=600 + N)
+    for nbins in (64, 1000, 4096):
+        hist, e_lo, width = B.ising_dos(J, h, nbins)
+        st = B.last_stats()
+        hist = hist.cpu().numpy().astype(np.uint64)
+        assert int(hist.sum()) == 1 << N and st.configs == 1 << N and st.kernel_variant == 2
+        want, outside = oracle.dos(J, h, e_lo, width, nbins)
+        assert outside == 0
+        if kind == "int":
+            assert st.exact and hist.tolist() == want.tolist()
+        else:
+            en = oracle.energies_range(J, h, 0, 1 << N)
+            frac = (en - e_lo) / width
+            near = np.abs(frac - np.rint(frac)) * width <= st.epsilon          # states that may legitimately move
+            moved = int(np.abs(hist.astype(np.int64) - want.astype(np.int64)).sum())
+            assert moved <= 2 * int(near.sum())
+            # and cumulative counts agree wherever no such state is near the edge
+            edges_with_near = set(np.rint(frac[near]).astype(int).tolist())
+            cg, cw = np.cumsum(hist.astype(np.int64)), np.cumsum(want.astype(np.int64))
+            for b in range(nbins - 1):
+                if (b + 1) not in edges_with_near:
+                    assert cg[b] == cw[b]
+
+
+def test_dos_ferromagnet_closed_form_30(B):
+    """2^30 states, binomial level counts (no oracle run needed)."""
+    from math import comb
+    N = 30
+    J, h = I.ferromagnet(N)
+    hist, e_lo, width = B.ising_dos(J, h, 4096)
+    hist = hist.cpu().numpy().astype(np.uint64)
+    assert int(hist.sum()) == 1 << N
+    got = {}
+    for b in np.nonzero(hist)[0]:
+        got[e_lo + b * width] = int(hist[b])
+    want = {}
+    for k in range(N // 2 + 1):
+        E = -((N - 2 * k) ** 2 - N) / 2
+        lo_edge = e_lo + np.floor((E - e_lo) / width) * width
+        want[lo_edge] = want.get(lo_edge, 0) + comb(N, k) * (1 if 2 * k == N else 2)
+    assert got == want

@@ -245,3 +245,28 @@ def test_gray_oracle_reproduces_config2_golden(golden_dir):
     qo, eo = load_golden(os.path.join(golden_dir, "cfg2.txt"))
     qg, eg = oracle.lowest_gray(c.J, c.h, len(qo), threads=2)
     assert qg.tolist() == qo.tolist() and eg.tolist() == eo.tolist()
+
+
+# ---------- density of states: closed-form level counts ----------
+def test_dos_binomial_levels():
+    from math import comb
+    N = 14
+    # uniform field h_i = 1, no couplings: E = -(N - 2k) for k spins down, C(N, k) states
+    hist, outside = oracle.dos(np.zeros((N, N)), np.ones(N), -N - 0.5, 1.0, 2 * N + 1)
+    assert outside == 0 and int(hist.sum()) == 1 << N
+    for k in range(N + 1):
+        assert int(hist[2 * k]) == comb(N, k)              # E = -N + 2k sits in bin 2k
+    assert not hist[1::2].any()
+    # uniform ferromagnet: E(k) = -((N-2k)^2 - N)/2 shared by k and N-k flipped spins
+    J, h = I.ferromagnet(N)
+    lo = -N * (N - 1) / 2
+    hist, outside = oracle.dos(J, h, lo - 0.5, 1.0, N * (N - 1) // 2 + N // 2 + 2)
+    assert outside == 0
+    for k in range(N // 2 + 1):
+        E = -((N - 2 * k) ** 2 - N) / 2
+        want = comb(N, k) * (1 if 2 * k == N else 2)
+        assert int(hist[int(E - lo)]) == want
+    assert int(hist.sum()) == 1 << N
+    # states below the first bin are reported, not counted
+    hist, outside = oracle.dos(J, h, lo + 0.5, 1.0, 4096)
+    assert outside == 2 and int(hist.sum()) == (1 << N) - 2
