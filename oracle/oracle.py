@@ -152,5 +152,43 @@ def lowest_gray(J, h, S: int, q_begin: int = 0, q_end: int | None = None, slab_b
     return states[:n].copy(), en[:n].copy()
 
 
+_SO_BNB = os.path.join(_HERE, "liboracle_bnb.so")
+_lib_bnb = None
+
+
+def build_bnb(force: bool = False) -> str:
+    """Compile oracle_bnb.c (tier-3 oracle: exact branch and bound; see its header)."""
+    src = os.path.join(_HERE, "oracle_bnb.c")
+    if force or not os.path.exists(_SO_BNB) or os.path.getmtime(_SO_BNB) < os.path.getmtime(src):
+        subprocess.check_call(["gcc", "-O2", "-fopenmp", "-fPIC", "-shared", "-ffp-contract=off", "-o", _SO_BNB, src, "-lm"])
+    return _SO_BNB
+
+
+def lowest_bnb(J, h, S: int, spare: int = 48, threads: int = 0):
+    """Tier-3 oracle: the S + spare lowest (E, q) of the whole space by exact branch and bound (fp64).
+    Pinned to `lowest` by tests/test_oracle_pins.py; used to write tests/golden/cfg5.txt.
+    Returns (states, energies, nodes_visited); the first S entries are the answer, the rest are spare."""
+    global _lib_bnb
+    if _lib_bnb is None:
+        build_bnb()
+        lib = ctypes.CDLL(_SO_BNB)
+        dp = ctypes.POINTER(ctypes.c_double)
+        up = ctypes.POINTER(ctypes.c_uint64)
+        lib.oracle_bnb_lowest.restype = ctypes.c_int64
+        lib.oracle_bnb_lowest.argtypes = [dp, dp, ctypes.c_int, ctypes.c_int64, ctypes.c_int64, up, dp, ctypes.c_int, up]
+        _lib_bnb = lib
+    J, h, N, Jp, hp = _prep(J, h)
+    K = S + spare
+    states = np.empty(K, dtype=np.uint64)
+    en = np.empty(K, dtype=np.float64)
+    nodes = ctypes.c_uint64(0)
+    n = _lib_bnb.oracle_bnb_lowest(Jp, hp, N, int(S), int(spare),
+                                   states.ctypes.data_as(ctypes.POINTER(ctypes.c_uint64)),
+                                   en.ctypes.data_as(ctypes.POINTER(ctypes.c_double)), int(threads), ctypes.byref(nodes))
+    if n < 0:
+        raise ValueError("oracle_bnb_lowest: bad arguments")
+    return states[:n].copy(), en[:n].copy(), int(nodes.value)
+
+
 def max_threads() -> int:
     return int(_load().oracle_max_threads())

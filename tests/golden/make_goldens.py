@@ -8,8 +8,9 @@ Each file cfg<k>.txt holds the oracle's S+16 lowest (q, E) pairs of BASELINE.jso
 under a second, config 2 minutes, config 3 about 2.6 hours on 8 cores with the plain oracle (oracle.c).
 Config 4 (2^40 states, integer weights) is out of reach of the plain oracle (about 40 hours) and is written
 by the tier-2 oracle oracle_gray.c (exact int64 single-spin-flip recurrence, pinned to oracle.c by
-tests/test_oracle_pins.py) in about half an hour; its file says so. Config 5 is out of reach of both
-(DESIGN.md "Parity status").
+tests/test_oracle_pins.py) in about an hour; its file says so. Config 5 (2^48 states, real weights) is out of
+reach of both and is written by the tier-3 oracle oracle_bnb.c (exact branch and bound in fp64, pinned to oracle.c
+by the same tests, including the stored lists of configs 1, 3 and 4) in seconds; its file says so.
 With --chunks C the state space is cut into C equal ranges of q; the oracle's S+16 lowest of each range
 (oracle_lowest on [q_begin, q_end)) are appended to tests/golden/.cfg<k>.partial as they finish, so an
 interrupted run resumes where it stopped; the union of the per-range lists is then ordered by (E, q) and cut
@@ -77,12 +78,16 @@ def main(argv):
         if chunks:
             q, e, dt = lowest_chunked(c, k, chunks)
         else:
-            q, e = (oracle.lowest_gray if k == 4 else oracle.lowest)(c.J, c.h, c.S + EXTRA)
+            if k == 5:
+                q, e, _nodes = oracle.lowest_bnb(c.J, c.h, c.S, spare=EXTRA)
+            else:
+                q, e = (oracle.lowest_gray if k == 4 else oracle.lowest)(c.J, c.h, c.S + EXTRA)
             dt = time.time() - t0
         path = os.path.join(HERE, f"cfg{k}.txt")
         with open(path, "w") as f:
             f.write(f"# BASELINE.json config {k}: {c.name}, N={c.N}, S={c.S} (+{EXTRA} spare)\n")
-            src = "oracle/oracle_gray.c (tier-2 oracle, integer instances)" if k == 4 else "oracle/oracle.c"
+            src = ("oracle/oracle_gray.c (tier-2 oracle, integer instances)" if k == 4 else
+                   "oracle/oracle_bnb.c (tier-3 oracle, exact branch and bound)" if k == 5 else "oracle/oracle.c")
             f.write(f"# written by tests/golden/make_goldens.py from {src} only; oracle wall time {dt:.1f} s, "
                     f"{oracle.max_threads()} threads\n")
             f.write(f"# instance sha256 {c.sha256()}\n")

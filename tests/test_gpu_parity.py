@@ -138,7 +138,7 @@ def test_config1_golden(B, golden_dir):
     assert_real(q, e, qo, eo, np.abs(np.triu(c.J, 1)).sum() + np.abs(c.h).sum(), c.S)
 
 
-@pytest.mark.parametrize("k", [2, 3, 4])
+@pytest.mark.parametrize("k", [2, 3, 4, 5])
 def test_config_golden(B, golden_dir, k):
     path = os.path.join(golden_dir, f"cfg{k}.txt")
     if not os.path.exists(path):

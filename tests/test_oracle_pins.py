@@ -270,3 +270,50 @@ def test_dos_binomial_levels():
     # states below the first bin are reported, not counted
     hist, outside = oracle.dos(J, h, lo + 0.5, 1.0, 4096)
     assert outside == 2 and int(hist.sum()) == (1 << N) - 2
+
+
+# ---------- tier-3 oracle (oracle_bnb.c, exact branch and bound) pinned to the plain oracle ----------
+@pytest.mark.parametrize("N,S,kind", [(1, 2, "real"), (4, 16, "real"), (9, 100, "real"), (14, 300, "real"), (18, 64, "real"),
+                                      (21, 1000, "real"), (24, 100, "real"), (12, 500, "int"), (20, 200, "int"),
+                                      (22, 300, "sparse"), (16, 65536, "real")])
+def test_bnb_oracle_equals_plain_oracle(N, S, kind):
+    if kind == "real":
+        J, h = I.complete_gaussian(N, seed=41 * N + S)
+    elif kind == "int":
+        J, h = I.random_integer(N, seed=43 * N, wmax=2, density=0.6)          # heavy ties: order decided by q
+    else:
+        J, h = I.random_integer(N, seed=47 * N, wmax=3, density=0.15)
+    qo, eo = oracle.lowest(J, h, S)
+    spare = min(16, (1 << N) - S)
+    for threads in (1, 4):
+        qb, eb, nodes = oracle.lowest_bnb(J, h, S, spare=spare, threads=threads)
+        assert len(qb) == S + spare and nodes > 0
+        assert qb[:S].tolist() == qo.tolist() and eb[:S].tolist() == eo.tolist()
+
+
+def test_bnb_oracle_closed_forms_and_goldens(golden_dir):
+    from checker import load_golden
+    # fields only, N = 40 (2^40 states: out of reach of the plain oracle): ground state and first excitation
+    N = 40
+    J, h = I.fields_only(N, seed=9)
+    qb, eb, _ = oracle.lowest_bnb(J, h, 2, spare=0)
+    q0 = sum(1 << i for i in range(N) if h[i] > 0)
+    w = int(np.argmin(np.abs(h)))
+    assert qb.tolist() == [q0, q0 ^ (1 << w)]
+    assert abs(eb[0] + np.abs(h).sum()) < 1e-12 and abs(eb[1] - eb[0] - 2 * abs(h[w])) < 1e-12
+    # Mattis N = 34: ground pair + the 2N one-flip states, ties by q
+    N = 34
+    J, h, xi = I.mattis(N, seed=11)
+    q_xi = sum(1 << i for i in range(N) if xi[i] > 0)
+    full = (1 << N) - 1
+    E0, E1 = -N * (N - 1) / 2, -((N - 2) ** 2 - N) / 2
+    exp = sorted([(E0, q_xi), (E0, full ^ q_xi)] + [(E1, q_xi ^ (1 << i)) for i in range(N)]
+                 + [(E1, full ^ q_xi ^ (1 << i)) for i in range(N)])
+    qb, eb, _ = oracle.lowest_bnb(J, h, len(exp), spare=0)
+    assert [(float(e), int(q)) for q, e in zip(qb, eb)] == exp
+    # the stored lists written by the plain oracle (configs 1, 3) and by the tier-2 oracle (config 4): S + 16 entries each
+    for k in (1, 3, 4):
+        c = I.baseline_config(k)
+        qo, eo = load_golden(os.path.join(golden_dir, f"cfg{k}.txt"))
+        qb, eb, _ = oracle.lowest_bnb(c.J, c.h, c.S, spare=16)
+        assert qb.tolist() == qo.tolist() and eb.tolist() == eo.tolist(), f"config {k}"
