@@ -26,6 +26,9 @@
  *                    Mattis closed forms, fields-only, chain, QUBO identity eqs. (2),(3), h=0 symmetry.
  *   oracle_lowest  : the same closed-form spectra incl. tie order, full sort for N <= 16,
  *                    decoupled-blocks pair-sum construction, range splitting.
+ *   oracle_dos     : binomial level counts (uniform field, uniform ferromagnet).
+ * Faster exact oracles for the configs this one cannot finish live in oracle_gray.c and oracle_bnb.c; both are
+ * pinned to this file and neither replaces it as the definition.
  */
 #include <stdint.h>
 #include <stdlib.h>
