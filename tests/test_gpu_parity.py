@@ -616,3 +616,13 @@ def test_dos_ferromagnet_closed_form_30(B):
         lo_edge = e_lo + np.floor((E - e_lo) / width) * width
         want[lo_edge] = want.get(lo_edge, 0) + comb(N, k) * (1 if 2 * k == N else 2)
     assert got == want
+
+
+@pytest.mark.parametrize("N,seed,S,hs", [(40, 4001, 300, 1.0), (42, 4201, 100, 0.5), (44, 4401, 1000, 1.0), (45, 4501, 64, 2.0)])
+def test_full_space_vs_branch_and_bound_oracle(B, N, seed, S, hs):
+    """Whole 2^N spaces the plain oracle cannot reach, against the tier-3 (branch and bound) oracle: bit-exact lists."""
+    J, h = I.complete_gaussian(N, seed=seed, h_scale=hs)
+    q, e = gpu_lowest(B, J, h, S)
+    assert B.last_stats().configs == 1 << N
+    qo, eo, _ = oracle.lowest_bnb(J, h, S, spare=16)
+    assert_exact(q, e, qo[:S], eo[:S])
