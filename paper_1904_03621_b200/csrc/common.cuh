@@ -93,7 +93,9 @@ struct Tables {
     //      2^shift16 grid units, every entry rounded DOWN (floor), so sums of them are lower bounds ----
     int shift16;                   // s: one 16-bit unit = 2^s grid units (0 for small-integer instances: exact)
     int cU16;                      // offset added to every 16-bit U entry so that it is never negative
-    unsigned Cp[(NMID / 2) * NLO]; // Cp[u][lo]  = pack( C[m0][lo] >> s , C[m0 | 8][lo] >> s ),  m0 = (u & 7) | ((u >> 3) << 4)
+    int cC16;                      // same for the C entries
+    int bV16;                      // same for the V entries (both register sets)
+    unsigned Cp[(NMID / 2) * NLO]; // Cp[u][lo]  = pack( (C[m0][lo] >> s) + cC , (C[m0 | 8][lo] >> s) + cC ),  m0 = (u & 7) | ((u >> 3) << 4)
     unsigned DVp[LW_MAX * 2 * NLO];        // DVp[k][sb][lo] = +-(DV[k][1][lo] >> s) * 65537    (both halves alike)
     unsigned DUp[LW_MAX * 2 * (NMID / 2)]; // DUp[k][sb][u]  = +-((DU[k][1][m0] >> s) + 65536 (DU[k][1][m0 | 8] >> s))
 };

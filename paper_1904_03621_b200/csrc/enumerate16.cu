@@ -201,6 +201,7 @@ enumerate16_kernel(const Tables* __restrict__ tab, Ctrl* __restrict__ ctrl, Entr
 
     const int s16 = tab->shift16;
     const int cU = tab->cU16;
+    const int bV = tab->bV16;
     unsigned Va[NLO], Vb[NLO], Up[NHALF];
     {
         // exact V[x] = QL[x] - 2 sum_{i in x} Phi_i by subset sums, then floor to 16-bit units and bias
@@ -214,8 +215,8 @@ enumerate16_kernel(const Tables* __restrict__ tab, Ctrl* __restrict__ ctrl, Entr
 #pragma unroll
         for (int x = 0; x < NLO; ++x) {
             const int v = acc[x] + tab->QL[x];
-            Va[x] = (unsigned)((v >> s16) + 32768) * 65537u;                           // mid bit 4 clear
-            Vb[x] = (unsigned)(((v + tab->C[16 * NLO + x]) >> s16) + 32768) * 65537u;  // mid bit 4 set
+            Va[x] = (unsigned)((v >> s16) + bV) * 65537u;                           // mid bit 4 clear
+            Vb[x] = (unsigned)(((v + tab->C[16 * NLO + x]) >> s16) + bV) * 65537u;  // mid bit 4 set
         }
         acc[0] = 0;
 #pragma unroll
@@ -236,7 +237,7 @@ enumerate16_kernel(const Tables* __restrict__ tab, Ctrl* __restrict__ ctrl, Entr
     const int tauE = ctrl->tauE;
     const unsigned long long tauQ = ctrl->tauQ;
     const unsigned long long q0_warp = q0 - ((unsigned long long)lane << nlow);
-    const int bias = 32768 + cU;
+    const int bias = bV + tab->cC16 + cU;
 
     const unsigned nsteps = 1u << Lw;
     for (unsigned t = 0; t < nsteps; ++t) {
@@ -278,12 +279,18 @@ enumerate16_kernel(const Tables* __restrict__ tab, Ctrl* __restrict__ ctrl, Entr
             // one row of C serves two register sets (mid bit 4 clear / set): 8 add-mins per LDS.128,
             // and the two chains are independent
             const uint4* crow = reinterpret_cast<const uint4*>(sCp + r * NLO);
-            unsigned ma = 0xffffffffu, mb = 0xffffffffu;
+            unsigned ma, mb;
 #pragma unroll
             for (int x = 0; x < NLO / 4; ++x) {
                 const uint4 c = crow[x];
-                ma = __viaddmin_u16x2(Va[4 * x + 0], c.x, ma);
-                mb = __viaddmin_u16x2(Vb[4 * x + 0], c.x, mb);
+                if (x == 0) {
+                    // the first sum of a row needs no minimum: a plain packed add (no half can wrap), FMA pipe
+                    ma = add_fma_pipe(Va[0], c.x);
+                    mb = add_fma_pipe(Vb[0], c.x);
+                } else {
+                    ma = __viaddmin_u16x2(Va[4 * x + 0], c.x, ma);
+                    mb = __viaddmin_u16x2(Vb[4 * x + 0], c.x, mb);
+                }
                 ma = __viaddmin_u16x2(Va[4 * x + 1], c.y, ma);
                 mb = __viaddmin_u16x2(Vb[4 * x + 1], c.y, mb);
                 ma = __viaddmin_u16x2(Va[4 * x + 2], c.z, ma);
@@ -291,8 +298,9 @@ enumerate16_kernel(const Tables* __restrict__ tab, Ctrl* __restrict__ ctrl, Entr
                 ma = __viaddmin_u16x2(Va[4 * x + 3], c.w, ma);
                 mb = __viaddmin_u16x2(Vb[4 * x + 3], c.w, mb);
             }
-            g = __viaddmin_u16x2(ma, Up[r], g);
-            g = __viaddmin_u16x2(mb, Up[r + NHALF / 2], g);
+            // fold both rows into g with ONE ALU instruction: the two packed sums cannot wrap (stage.cu), so they are
+            // plain 32-bit adds on the FMA pipe, and VIMNMX3 takes the minimum of the three
+            g = __vimin3_u16x2(g, add_fma_pipe(ma, Up[r]), add_fma_pipe(mb, Up[r + NHALF / 2]));
         }
         // ---- a4: threshold filter on the lower bound:  bound * 2^s + Eh <= tauE  <=>  bound <= (tauE - Eh) >> s ----
         const int gm = (int)min(g & 0xffffu, g >> 16) - bias;

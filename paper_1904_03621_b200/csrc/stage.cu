@@ -206,8 +206,11 @@ __global__ void __launch_bounds__(256) tables_kernel(Tables* __restrict__ tab, C
     //   |V| <= BV = max|QL| + 2 sum_{i in lo} R_i,  |U| <= BU = max|QM| + 2 sum_{i in mid} R_i,  |C| <= BC = max|C|.
     // A quantised entry is off by less than 1 unit, a walked table by less than 1 + LW_MAX units (one floor per
     // set walk bit). s is the smallest shift for which no 16-bit lane can wrap (see enumerate16.cu header):
-    //   X16 = (BX >> s) + 2 + LW_MAX,   cU = U16,   V16 + C16 + 2 cU <= 32767.
-    __shared__ int s_shift, s_cU;
+    // Every packed half is stored with an offset that makes it non-negative (so that packed words can be added with
+    // plain 32-bit adds): V + bV, C + cC, U + cU with
+    //   cC = (BC >> s) + 2,  cU = (BU >> s) + 2 + LW_MAX,  bV = (BV >> s) + 2 + LW_MAX + cC   (register set b holds
+    //   V + C[16][.], hence the extra cC);  the largest half a sum can reach is 2 (bV + cC + cU) <= 65535.
+    __shared__ int s_shift, s_cU, s_cC;
     __syncthreads();                                   // QL, QM, C above are complete
     if (tid == 0) {
         long long BV = 0, BU = 0, BC = 0, m;
@@ -220,14 +223,20 @@ __global__ void __launch_bounds__(256) tables_kernel(Tables* __restrict__ tab, C
             if (i < LL) BV += 2 * R; else BU += 2 * R;
         }
         int s = 0;
+        long long cC = 0, cU = 0, bV = 0;
         for (; s < 40; ++s) {
-            const long long V16 = (BV >> s) + 2 + LW_MAX, U16 = (BU >> s) + 2 + LW_MAX, C16 = (BC >> s) + 2;
-            if (V16 + C16 + 2 * U16 <= 32767) break;
+            cC = (BC >> s) + 2;
+            cU = (BU >> s) + 2 + LW_MAX;
+            bV = (BV >> s) + 2 + LW_MAX + cC;
+            if (2 * (bV + cC + cU) <= 65535) break;
         }
         s_shift = s;
-        s_cU = (int)((BU >> s) + 2 + LW_MAX);
+        s_cU = (int)cU;
+        s_cC = (int)cC;
         tab->shift16 = s;
-        tab->cU16 = s_cU;
+        tab->cU16 = (int)cU;
+        tab->cC16 = (int)cC;
+        tab->bV16 = (int)bV;
         ctrl->shift16 = s;
     }
     __syncthreads();
@@ -237,8 +246,8 @@ __global__ void __launch_bounds__(256) tables_kernel(Tables* __restrict__ tab, C
     for (int idx = tid; idx < (NMID / 2) * NLO; idx += blockDim.x) {
         const int u = idx / NLO, lo = idx % NLO;
         const int m0 = (u & 7) | ((u >> 3) << 4);
-        const int a = tab->C[m0 * NLO + lo] >> s16, b = tab->C[(m0 | 8) * NLO + lo] >> s16;
-        tab->Cp[idx] = ((unsigned)a & 0xffffu) | ((unsigned)b << 16);
+        const int a = (tab->C[m0 * NLO + lo] >> s16) + s_cC, b = (tab->C[(m0 | 8) * NLO + lo] >> s16) + s_cC;
+        tab->Cp[idx] = (unsigned)a + ((unsigned)b << 16);        // both halves non-negative
     }
     for (int idx = tid; idx < LW_MAX * NLO; idx += blockDim.x) {
         const int k = idx / NLO, lo = idx % NLO;
