@@ -33,8 +33,13 @@ UNIT = "configs/s"
 # integer-ALU ceiling of the inner operation: VIADDMNMX issues on the ALU pipe at
 # 148 SMs x 4 sub-partitions x 16 lanes/clk (B300_MICROARCH.md "Pipe rates") x 1.965 GHz (MEASURED_PEAKS.json);
 # the default kernel's VIADDMNMX.U16x2 forms two 16-bit add-mins (two configurations) per lane instruction,
-# the int32 kernel (ISING_KERNEL=32) one.
+# the int32 kernel (ISING_KERNEL=32) one. The default kernel also forms part of its sums as packed adds on the FMA
+# pipe and takes the minimum of two of them with one VIMNMX3.U16x2 (4 configurations per ALU lane instruction, 3 issue
+# slots); with the ALU pipe at 16 lanes/clk and one warp instruction issued per clock per sub-partition the best
+# possible mix of the two forms is 48 configurations/clk/sub-partition = 192 per SM: that bound is
+# `roofline.peak`; the ceiling of the fused form alone (128 per SM) is reported beside it.
 ALU_LANES_PER_CLK_PER_SM = 64
+MIX_BOUND_CONFIGS_PER_CLK_PER_SM = 192
 FMA_LANES_PER_CLK_PER_SM = 128
 
 
@@ -301,8 +306,13 @@ def main():
             pass
         sms = torch.cuda.get_device_properties(local_rank).multi_processor_count
         per_inst = 2 if st.kernel_variant == 16 else 1                 # add-mins (configurations) per lane instruction
-        alu_peak = sms * ALU_LANES_PER_CLK_PER_SM * sm_max_hz * per_inst          # add-min ops / s
-        live_peak = addmin16x2_peak * 2 if st.kernel_variant == 16 else addmin_peak
+        fused_peak = sms * ALU_LANES_PER_CLK_PER_SM * sm_max_hz * per_inst         # add-min ops / s, fused form only
+        fused_live = addmin16x2_peak * 2 if st.kernel_variant == 16 else addmin_peak
+        if st.kernel_variant == 16:
+            alu_peak = sms * MIX_BOUND_CONFIGS_PER_CLK_PER_SM * sm_max_hz
+            live_peak = fused_live * MIX_BOUND_CONFIGS_PER_CLK_PER_SM / (ALU_LANES_PER_CLK_PER_SM * per_inst)
+        else:
+            alu_peak, live_peak = fused_peak, fused_live
         kname = "ising::enumerate16_kernel" if st.kernel_variant == 16 else "ising::enumerate_kernel"
         fma_nominal = sms * FMA_LANES_PER_CLK_PER_SM * sm_max_hz       # FMA / s
         achieved = float(enum_configs) / (enum_ms * 1e-3)   # this rank's kernel: one add-min per configuration
@@ -336,9 +346,15 @@ def main():
                          "frac": achieved / alu_peak, "traffic": traffic,
                          "kernel": kname, "launches": enum_launches,
                          "avg_launch_ms": enum_ms / max(enum_launches, 1),
-                         "peak_source": f"derived: SMs x 64 ALU lanes/clk x {per_inst} add-min per lane instruction "
-                                        "x sm_max_mhz of MEASURED_PEAKS.json (DESIGN.md 5.2)",
+                         "peak_source": ("derived: SMs x 192 add-min/clk (ALU pipe 16 lanes/clk and 1 issue slot/clk per "
+                                         "sub-partition; best mix of VIADDMNMX.U16x2 and IMAD+IMAD+VIMNMX3.U16x2) "
+                                         "x sm_max_mhz of MEASURED_PEAKS.json (DESIGN.md 5.2)"
+                                         if st.kernel_variant == 16 else
+                                         "derived: SMs x 64 ALU lanes/clk x 1 add-min per lane instruction "
+                                         "x sm_max_mhz of MEASURED_PEAKS.json (DESIGN.md 5.2)"),
                          "peak_measured_live": live_peak, "frac_of_measured_live": achieved / live_peak,
+                         "fused_only_ceiling": fused_peak, "frac_of_fused_only_ceiling": achieved / fused_peak,
+                         "fused_only_ceiling_measured_live": fused_live,
                          "viaddmnmx_s32_per_s_live": addmin_peak, "viaddmnmx_u16x2_per_s_live": addmin16x2_peak},
             "gpu_launches": launches,
             "clocks": clocks,

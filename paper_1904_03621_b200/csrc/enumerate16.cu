@@ -5,22 +5,30 @@
 // fixed point: one unit = 2^s grid units, every table entry rounded DOWN, so that
 //      V16[lo] + C16[mid][lo] + U16[mid]  <=  (V[lo] + C[mid][lo] + U[mid]) / 2^s            (a rigorous lower bound)
 // and the inner operation  m = min(V16 + C16, m)  is one VIADDMNMX.U16x2 for the two configurations (lo, mid) and
-// (lo, mid | 8): 512 + 16 ALU instructions per 1024 configurations instead of 1024 + 32. A block whose bound is
+// (lo, mid | 8): about 450 ALU instructions per 1024 configurations instead of 1024 + 32. A block whose bound is
 // <= tau is formed again by the whole warp in exact int32 grid arithmetic (the same a4 path as enumerate.cu), so
 // what reaches the pool -- and everything after it -- is identical to the int32 kernel; the 16-bit screen can only
 // cause extra (false) hits, never a miss. For integer instances with small weights s = 0 and the screen is exact.
 //
-// Representation (so that no 16-bit lane ever wraps, stage.cu chooses s accordingly); m0(u) = (u & 7) | ((u >> 3) << 4):
-//   Va[lo]  both halves = V16[lo] + 32768                       (biased, in [0, 65535]); mid bit 4 clear
-//   Vb[lo]  both halves = floor((V[lo] + C[16][lo]) / 2^s) + 32768                       mid bit 4 set
-//   Cp[u][lo] = ( C16[m0(u)][lo] , C16[m0(u) | 8][lo] )         (two's complement halves; the lane add is mod 2^16)
-//   Up[u]   = ( U16[m0(u)] + cU , U16[m0(u) | 8] + cU )         (offset cU >= |U16|: non-negative halves)
-//   block bound = min over halves of g  -  32768 - cU
+// Representation (stage.cu chooses s so that no 16-bit half ever wraps and every half is a NON-NEGATIVE number);
+// m0(u) = (u & 7) | ((u >> 3) << 4):
+//   Va[lo]  both halves = V16[lo] + bV                                             mid bit 4 clear
+//   Vb[lo]  both halves = floor((V[lo] + C[16][lo]) / 2^s) + bV                    mid bit 4 set
+//   Cp[u][lo] = ( C16[m0(u)][lo] + cC , C16[m0(u) | 8][lo] + cC )
+//   Up[u]   = ( U16[m0(u)] + cU , U16[m0(u) | 8] + cU )
+//   block bound = min over halves of g  -  (bV + cC + cU)
 // The two halves of a word differ in mid bit 3; mid bit 4 is resolved by the two register sets Va / Vb, which both
 // consume the SAME row of Cp (rows u < 8 only): one warp-uniform LDS.128 feeds 8 add-mins.
-// Because every half of Va, Vb and Up is a non-negative number that stays inside its 16 bits, a Gray step may update
-// the packed words with plain 32-bit integer adds of the packed delta (d_lo + 65536 d_hi): those run as IMAD on the
-// FMA pipe, off the ALU pipe that bounds the kernel.
+// Because every half is non-negative and stays inside its 16 bits, a packed sum is also a plain 32-bit integer add.
+// That is used three times to take work off the ALU pipe, which bounds the kernel (adds issue as IMAD x*1+y on the
+// FMA pipe):
+//   * a Gray step updates the packed tables with 32-bit adds of the packed delta (d_lo + 65536 d_hi);
+//   * the first sum of every row and the two sums of every row fold are plain adds; the fold's minimum of three is
+//     ONE VIMNMX3.U16x2;
+//   * in the last P1_CHUNKS of the 8 chunks of a row the sums are plain adds and one VIMNMX3.U16x2 takes the minimum
+//     of two of them: 4 configurations per ALU instruction instead of 2, for one more issue slot per two sums.
+//     Measured on B200 (2^45-state slice of cfg5): P1_CHUNKS = 0: 3.25e13/s, 1: 3.39e13, 2: 3.42e13, 3: 3.41e13,
+//     4: 3.41e13, 5: 3.29e13 -- beyond 2 the issue slots, not the ALU pipe, become the limit.
 //
 // Walk: as in enumerate.cu (reflected Gray code over the Lw walk bits). The walked 16-bit tables are
 // V16 = floor(V(q0)/2^s) + sum over SET walk bits k of floor(DV_on[k]/2^s): turning a bit off subtracts exactly what
@@ -39,6 +47,9 @@ namespace ising {
 
 constexpr int E16_THREADS = 256;
 constexpr int NHALF = NMID / 2;
+#ifndef P1_CHUNKS
+#define P1_CHUNKS 2
+#endif
 
 static_assert(LL == 5 && LM == 5, "the subset-sum unrolling below assumes 5 lo and 5 mid bits");
 
@@ -287,16 +298,33 @@ enumerate16_kernel(const Tables* __restrict__ tab, Ctrl* __restrict__ ctrl, Entr
                     // the first sum of a row needs no minimum: a plain packed add (no half can wrap), FMA pipe
                     ma = add_fma_pipe(Va[0], c.x);
                     mb = add_fma_pipe(Vb[0], c.x);
+                    ma = __viaddmin_u16x2(Va[1], c.y, ma);
+                    mb = __viaddmin_u16x2(Vb[1], c.y, mb);
+                    ma = __viaddmin_u16x2(Va[2], c.z, ma);
+                    mb = __viaddmin_u16x2(Vb[2], c.z, mb);
+                    ma = __viaddmin_u16x2(Va[3], c.w, ma);
+                    mb = __viaddmin_u16x2(Vb[3], c.w, mb);
+                } else if (x >= NLO / 4 - P1_CHUNKS) {
+                    // pipe balancing: these sums are formed as plain packed adds on the FMA pipe and one VIMNMX3
+                    // takes the minimum of two of them -- half the ALU-pipe time, one more issue slot per two sums
+                    const unsigned a0 = add_fma_pipe(Va[4 * x + 0], c.x), b0 = add_fma_pipe(Vb[4 * x + 0], c.x);
+                    const unsigned a1 = add_fma_pipe(Va[4 * x + 1], c.y), b1 = add_fma_pipe(Vb[4 * x + 1], c.y);
+                    const unsigned a2 = add_fma_pipe(Va[4 * x + 2], c.z), b2 = add_fma_pipe(Vb[4 * x + 2], c.z);
+                    const unsigned a3 = add_fma_pipe(Va[4 * x + 3], c.w), b3 = add_fma_pipe(Vb[4 * x + 3], c.w);
+                    ma = __vimin3_u16x2(ma, a0, a1);
+                    mb = __vimin3_u16x2(mb, b0, b1);
+                    ma = __vimin3_u16x2(ma, a2, a3);
+                    mb = __vimin3_u16x2(mb, b2, b3);
                 } else {
                     ma = __viaddmin_u16x2(Va[4 * x + 0], c.x, ma);
                     mb = __viaddmin_u16x2(Vb[4 * x + 0], c.x, mb);
+                    ma = __viaddmin_u16x2(Va[4 * x + 1], c.y, ma);
+                    mb = __viaddmin_u16x2(Vb[4 * x + 1], c.y, mb);
+                    ma = __viaddmin_u16x2(Va[4 * x + 2], c.z, ma);
+                    mb = __viaddmin_u16x2(Vb[4 * x + 2], c.z, mb);
+                    ma = __viaddmin_u16x2(Va[4 * x + 3], c.w, ma);
+                    mb = __viaddmin_u16x2(Vb[4 * x + 3], c.w, mb);
                 }
-                ma = __viaddmin_u16x2(Va[4 * x + 1], c.y, ma);
-                mb = __viaddmin_u16x2(Vb[4 * x + 1], c.y, mb);
-                ma = __viaddmin_u16x2(Va[4 * x + 2], c.z, ma);
-                mb = __viaddmin_u16x2(Vb[4 * x + 2], c.z, mb);
-                ma = __viaddmin_u16x2(Va[4 * x + 3], c.w, ma);
-                mb = __viaddmin_u16x2(Vb[4 * x + 3], c.w, mb);
             }
             // fold both rows into g with ONE ALU instruction: the two packed sums cannot wrap (stage.cu), so they are
             // plain 32-bit adds on the FMA pipe, and VIMNMX3 takes the minimum of the three
