@@ -210,7 +210,7 @@ __global__ void __launch_bounds__(256) tables_kernel(Tables* __restrict__ tab, C
     // plain 32-bit adds): V + bV, C + cC, U + cU with
     //   cC = (BC >> s) + 2,  cU = (BU >> s) + 2 + LW_MAX,  bV = (BV >> s) + 2 + LW_MAX + cC   (register set b holds
     //   V + C[16][.], hence the extra cC);  the largest half a sum can reach is 2 (bV + cC + cU) <= 65535.
-    __shared__ int s_shift, s_cU, s_cC;
+    __shared__ int s_shift, s_cC;
     __syncthreads();                                   // QL, QM, C above are complete
     if (tid == 0) {
         long long BV = 0, BU = 0, BC = 0, m;
@@ -231,7 +231,6 @@ __global__ void __launch_bounds__(256) tables_kernel(Tables* __restrict__ tab, C
             if (2 * (bV + cC + cU) <= 65535) break;
         }
         s_shift = s;
-        s_cU = (int)cU;
         s_cC = (int)cC;
         tab->shift16 = s;
         tab->cU16 = (int)cU;
