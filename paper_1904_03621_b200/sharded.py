@@ -42,13 +42,15 @@ def local_quota(S: int, q_begin: int, q_end: int) -> int:
 
 
 def ising_lowest_sharded(J, h, S: int, group=None, solver: Optional[Callable] = None,
-                         merger: Optional[Callable] = None, device=None):
+                         merger: Optional[Callable] = None, device=None, always_exchange: bool = False):
     """The S lowest (E, q) of the whole space, computed by all ranks of `group` together.
 
     J, h: the instance (identical on every rank). Returns (states, energies) tensors of length S on every rank.
     solver(J, h, S_local, q_begin, q_end) -> (states int64[S_local], energies float64[S_local]) tensors;
     merger(states int64[n], energies float64[n], S) -> (states[S], energies[S]).
     Defaults: the C-ABI calls `binding.ising_lowest_range` / `binding.ising_merge_lists` (CUDA; no CPU fallback).
+    always_exchange: run the all-gather and the merge even with a single rank (exercises the collective path on a
+    one-GPU box).
     """
     import torch
     import torch.distributed as dist
@@ -72,7 +74,7 @@ def ising_lowest_sharded(J, h, S: int, group=None, solver: Optional[Callable] = 
         dev = torch.device(device) if device is not None else torch.device("cpu")
         st = torch.empty(0, dtype=torch.int64, device=dev)
         en = torch.empty(0, dtype=torch.float64, device=dev)
-    if world == 1:
+    if world == 1 and not (always_exchange and dist.is_initialized()):
         return st, en
     # fixed-size exchange: every rank sends S slots, the unused tail is cut off again by the known quotas
     send_q = torch.zeros(S, dtype=torch.int64, device=dev)

@@ -626,3 +626,23 @@ def test_full_space_vs_branch_and_bound_oracle(B, N, seed, S, hs):
     assert B.last_stats().configs == 1 << N
     qo, eo, _ = oracle.lowest_bnb(J, h, S, spare=16)
     assert_exact(q, e, qo[:S], eo[:S])
+
+
+def test_sharded_exchange_path_over_nccl_single_rank(B):
+    """The all-gather + ising_merge_lists path of sharded.py on CUDA tensors over NCCL (world size 1: one GPU here)."""
+    import torch
+    import torch.distributed as dist
+    from paper_1904_03621_b200 import sharded
+    os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+    os.environ.setdefault("MASTER_PORT", "29533")
+    created = not dist.is_initialized()
+    if created:
+        dist.init_process_group("nccl", rank=0, world_size=1, device_id=torch.device("cuda", 0))
+    try:
+        c = I.baseline_config(3)
+        q, e = sharded.ising_lowest_sharded(c.J, c.h, c.S, always_exchange=True)
+        q0, e0 = B.ising_lowest(c.J, c.h, c.S)
+        assert q.is_cuda and torch.equal(q, q0) and torch.equal(e, e0)
+    finally:
+        if created:
+            dist.destroy_process_group()
