@@ -190,6 +190,13 @@ int ising_addmin_peak(double ms_target, double *addmin_per_s_out_host, void *str
  * ceiling of the packed kernel is twice this number. */
 int ising_addmin16x2_peak(double ms_target, double *inst_per_s_out_host, void *stream);
 
+/* The instruction MIX the default kernel is built from, register-only: per chain step one fused VIADDMNMX.U16x2
+ * (two 16-bit add-mins, ALU pipe) and one split group IMAD + IMAD + VIMNMX3.U16x2 (four add-mins: two packed sums on
+ * the FMA pipe, one three-way packed minimum on the ALU pipe). Writes lane ADD-MINS per second, whole GPU: the
+ * measured counterpart of the derived bound of DESIGN.md 5.2 (192 add-mins per clock per SM) and the denominator of
+ * bench.py's `roofline.peak`. */
+int ising_addmin_mix_peak(double ms_target, double *addmin_per_s_out_host, void *stream);
+
 /* Frees the calling thread's cached workspace (device pool, tables, pinned control block). Optional. */
 void ising_release_workspace(void);
 

@@ -22,7 +22,8 @@ S_MAX = 65536
 # every symbol include/ising.h declares (tests/test_abi.py checks the header against this list and the .so)
 EXPORTS = ["ising_lowest", "ising_lowest_range", "ising_lowest_host", "ising_lowest_h0", "ising_lowest_alg1", "ising_dos", "ising_merge_lists", "qubo_lowest",
            "ising_energies", "ising_get_last_stats", "ising_strerror", "ising_last_error", "ising_version",
-           "ising_fma_peak", "ising_addmin_peak", "ising_addmin16x2_peak", "ising_release_workspace"]
+           "ising_fma_peak", "ising_addmin_peak", "ising_addmin16x2_peak", "ising_addmin_mix_peak",
+           "ising_release_workspace"]
 
 
 class IsingError(RuntimeError):
@@ -94,6 +95,8 @@ def load():
     lib.ising_fma_peak.argtypes = [ctypes.c_double, ctypes.POINTER(ctypes.c_double), vp]
     lib.ising_addmin_peak.argtypes = [ctypes.c_double, ctypes.POINTER(ctypes.c_double), vp]
     lib.ising_addmin16x2_peak.argtypes = [ctypes.c_double, ctypes.POINTER(ctypes.c_double), vp]
+    lib.ising_addmin_mix_peak.argtypes = [ctypes.c_double, ctypes.POINTER(ctypes.c_double), vp]
+    lib.ising_addmin_mix_peak.restype = ctypes.c_int
     for name in ("ising_lowest", "ising_lowest_range", "ising_lowest_host", "ising_merge_lists", "qubo_lowest",
                  "ising_energies", "ising_get_last_stats", "ising_fma_peak", "ising_addmin_peak", "ising_addmin16x2_peak",
                  "ising_version"):
@@ -337,6 +340,13 @@ def addmin16x2_peak(ms_target: float = 50.0, stream=None) -> float:
     """VIADDMNMX.U16x2 lane instructions per second (two 16-bit add-mins each)."""
     v = ctypes.c_double(0.0)
     _check(load().ising_addmin16x2_peak(float(ms_target), ctypes.byref(v), _stream(stream)), "ising_addmin16x2_peak")
+    return v.value
+
+
+def addmin_mix_peak(ms_target: float = 50.0, stream=None) -> float:
+    """Lane add-mins per second of the fused + split instruction mix (include/ising.h)."""
+    v = ctypes.c_double(0.0)
+    _check(load().ising_addmin_mix_peak(float(ms_target), ctypes.byref(v), _stream(stream)), "ising_addmin_mix_peak")
     return v.value
 
 

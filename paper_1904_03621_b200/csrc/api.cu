@@ -7,6 +7,7 @@
 #include <cstring>
 #include <string>
 #include <vector>
+#include <climits>
 
 #include "common.cuh"
 #include "../../include/ising.h"
@@ -19,10 +20,13 @@ thread_local ising_stats t_stats;
 thread_local bool t_have_stats = false;
 
 // Per-host-thread, per-device scratch. Calls of one thread are sequential (each call synchronises its stream
-// before returning), so the workspace can be reused; different threads own different workspaces.
+// before returning), so the workspace can be reused; different threads own different workspaces. Freed when the
+// thread exits (or by ising_release_workspace); a partly failed allocation is freed before the error is returned.
 struct Workspace {
     int device = -1;
-    Entry* pool = nullptr;          // POOL_CAP entries
+    Entry* pool = nullptr;          // POOL_CAP entries: candidates
+    Entry* pool2 = nullptr;         // POOL_CAP entries: compacted candidates / band-pass scratch
+    unsigned* hist = nullptr;       // HIST_WORDS counters: candidate histogram (walk.cuh)
     Tables* tab = nullptr;
     Ctrl* ctrl = nullptr;
     Ctrl* h_ctrl = nullptr;         // pinned
@@ -33,12 +37,16 @@ struct Workspace {
     cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
     void release()
     {
-        if (device < 0) return;
-        cudaFree(pool); cudaFree(tab); cudaFree(ctrl); cudaFree(J2); cudaFree(h2); cudaFree(out_q); cudaFree(out_e);
+        cudaFree(pool); cudaFree(pool2); cudaFree(hist); cudaFree(tab); cudaFree(ctrl); cudaFree(J2); cudaFree(h2);
+        cudaFree(out_q); cudaFree(out_e);
         if (h_ctrl) cudaFreeHost(h_ctrl);
         for (auto& e : ev) if (e) cudaEventDestroy(e);
-        *this = Workspace();
+        pool = pool2 = nullptr; hist = nullptr; tab = nullptr; ctrl = h_ctrl = nullptr; J2 = h2 = nullptr;
+        out_q = nullptr; out_e = nullptr;
+        for (auto& e : ev) e = nullptr;
+        device = -1;
     }
+    ~Workspace() { if (device >= 0) release(); }
 };
 thread_local Workspace t_ws;
 
@@ -51,21 +59,43 @@ thread_local Workspace t_ws;
         }                                                                                           \
     } while (0)
 
+// after a kernel launch: a failed launch is reported at once, under the kernel's name
+#define LAUNCH_CHECK(name)                                                                          \
+    do {                                                                                            \
+        cudaError_t err__ = cudaGetLastError();                                                     \
+        if (err__ != cudaSuccess) {                                                                 \
+            t_last_error = std::string("launch of ") + (name) + ": " + cudaGetErrorString(err__);   \
+            return ISING_ERR_CUDA;                                                                  \
+        }                                                                                           \
+    } while (0)
+
+int allocate_workspace(Workspace& ws, int dev)
+{
+    CUDA_TRY(cudaMalloc(&ws.pool, sizeof(Entry) * (size_t)POOL_CAP));
+    CUDA_TRY(cudaMalloc(&ws.pool2, sizeof(Entry) * (size_t)POOL_CAP));
+    CUDA_TRY(cudaMalloc(&ws.hist, sizeof(unsigned) * (size_t)HIST_WORDS));
+    CUDA_TRY(cudaMalloc(&ws.tab, sizeof(Tables)));
+    CUDA_TRY(cudaMalloc(&ws.ctrl, sizeof(Ctrl)));
+    CUDA_TRY(cudaMallocHost(&ws.h_ctrl, sizeof(Ctrl)));
+    CUDA_TRY(cudaMalloc(&ws.J2, sizeof(double) * 64 * 64));
+    CUDA_TRY(cudaMalloc(&ws.h2, sizeof(double) * 64));
+    CUDA_TRY(cudaMalloc(&ws.out_q, sizeof(unsigned long long) * ISING_S_MAX));
+    CUDA_TRY(cudaMalloc(&ws.out_e, sizeof(double) * ISING_S_MAX));
+    for (auto& e : ws.ev) CUDA_TRY(cudaEventCreate(&e));
+    (void)dev;
+    set_select_attributes();                       // per-device function attributes (dynamic shared memory)
+    CUDA_TRY(cudaGetLastError());
+    return ISING_OK;
+}
+
 int ensure_workspace()
 {
     int dev = -1;
     CUDA_TRY(cudaGetDevice(&dev));
     if (t_ws.device == dev) return ISING_OK;
     t_ws.release();
-    CUDA_TRY(cudaMalloc(&t_ws.pool, sizeof(Entry) * (size_t)POOL_CAP));
-    CUDA_TRY(cudaMalloc(&t_ws.tab, sizeof(Tables)));
-    CUDA_TRY(cudaMalloc(&t_ws.ctrl, sizeof(Ctrl)));
-    CUDA_TRY(cudaMallocHost(&t_ws.h_ctrl, sizeof(Ctrl)));
-    CUDA_TRY(cudaMalloc(&t_ws.J2, sizeof(double) * 64 * 64));
-    CUDA_TRY(cudaMalloc(&t_ws.h2, sizeof(double) * 64));
-    CUDA_TRY(cudaMalloc(&t_ws.out_q, sizeof(unsigned long long) * ISING_S_MAX));
-    CUDA_TRY(cudaMalloc(&t_ws.out_e, sizeof(double) * ISING_S_MAX));
-    for (auto& e : t_ws.ev) CUDA_TRY(cudaEventCreate(&e));
+    const int rc = allocate_workspace(t_ws, dev);
+    if (rc != ISING_OK) { t_ws.release(); return rc; }
     t_ws.device = dev;
     return ISING_OK;
 }
@@ -85,14 +115,310 @@ int env_int(const char* name, int dflt, int lo, int hi)
     return v < lo ? lo : (v > hi ? hi : v);
 }
 
-__global__ void reset_count_kernel(Ctrl* ctrl) { ctrl->count = ctrl->kept; }
+// host-sequenced path: between launches
+__global__ void reset_queue_kernel(Ctrl* ctrl, int drop_new)
+{
+    ctrl->next_unit = 0ull;
+    ctrl->done_configs = 0ull;
+    if (drop_new) { ctrl->count = ctrl->kept; ctrl->pool_overflow = 0u; }
+}
+// restart of a whole run (after a void single-pass attempt) or start of the band pass
+__global__ void restart_kernel(Ctrl* ctrl, unsigned long long tau)
+{
+    ctrl->next_unit = 0ull;
+    ctrl->done_configs = 0ull;
+    ctrl->count = 0u;
+    ctrl->kept = 0u;
+    ctrl->pool_overflow = 0u;
+    ctrl->band_overflow = 0u;
+    ctrl->count2 = 0u;
+    ctrl->final_state = 0u;
+    ctrl->tau = tau;
+}
+// band pass: the sure states (grid energy below the band; a sorted prefix of pool) move to pool2, keyed by fp64 energy
+__global__ void count_sure_kernel(const Entry* __restrict__ pool, Ctrl* __restrict__ ctrl, unsigned kept, int band)
+{
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    const unsigned long long klim = key_from_i32(ctrl->eS - band);       // sure: key < klim
+    unsigned lo = 0, hi = kept;
+    while (lo < hi) {
+        const unsigned mid = (lo + hi) >> 1;
+        if (pool[mid].key < klim) lo = mid + 1; else hi = mid;
+    }
+    ctrl->n_sure = lo;
+}
+__global__ void copy_entries_kernel(const Entry* __restrict__ src, Entry* __restrict__ dst, unsigned n)
+{
+    const unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) dst[i] = src[i];
+}
+
+// One call's invariants, shared by the three host paths below.
+struct Run {
+    Workspace* ws;
+    ising_stats* stats;
+    const double *J, *h, *Jorig, *horig;
+    int mode, N, S, variant, lw_max, chunk_log2, growth, qshift;
+    unsigned keep_cap;
+    unsigned long long q_begin, q_end;
+    cudaStream_t st;
+    double enum_ms;
+};
+
+void plan_header(const Run& r, Plan& plan, int use_hist, int loE)
+{
+    memset(&plan, 0, sizeof(plan));
+    plan.q_begin = r.q_begin;
+    plan.q_end = r.q_end;
+    plan.N = r.N;
+    plan.S = r.S;
+    plan.use_hist = use_hist;
+    const int rf = r.S / 8;
+    plan.refresh = rf < 64 ? 64 : rf;
+    plan.qshift = r.qshift;
+    plan.loE = loE;
+    plan.keep_cap = r.keep_cap;
+}
+
+// Walk-bit count of a segment of sz configurations at cur: enough units to balance the persistent warps, aligned.
+int choose_lw(unsigned long long cur, unsigned long long sz, int lw_max)
+{
+    int Lw = floor_log2(sz) - MIN_CHUNK_BITS - 12;
+    Lw = Lw < 0 ? 0 : (Lw > lw_max ? lw_max : Lw);
+    while (Lw > 0 && (cur & ((1ull << (MIN_CHUNK_BITS + Lw)) - 1ull))) --Lw;
+    return Lw;
+}
+
+int launch_walk(const Run& r, const Plan& plan)
+{
+    Workspace& ws = *r.ws;
+    if (plan.total_units > 0x7fffffffull * WALK_WARPS) { t_last_error = "internal: too many units in one launch"; return ISING_ERR_INTERNAL; }
+    if (r.variant == 16) launch_walk16(ws.tab, ws.ctrl, ws.pool, ws.hist, plan, r.st);
+    else launch_walk32(ws.tab, ws.ctrl, ws.pool, ws.hist, plan, r.st);
+    LAUNCH_CHECK(r.variant == 16 ? "walk_kernel<Inner16>" : "walk_kernel<Inner32>");
+    r.stats->kernel_launches += 1;
+    r.stats->enum_launches += 1;
+    return ISING_OK;
+}
+
+int read_ctrl(const Run& r)
+{
+    CUDA_TRY(cudaMemcpyAsync(r.ws->h_ctrl, r.ws->ctrl, sizeof(Ctrl), cudaMemcpyDeviceToHost, r.st));
+    CUDA_TRY(cudaStreamSynchronize(r.st));
+    return ISING_OK;
+}
+
+// ---- single-pass path: ONE launch of the persistent kernel over the whole range (ramp-up segments, threshold
+// refreshed on the device), then compaction and the one-block final selection; one host synchronisation at the end.
+// Returns ISING_OK with *redo = true if the candidate pool overflowed (the run is void). ----
+int run_single_pass(Run& r, unsigned long long* states_out, double* energies_out, bool* redo)
+{
+    Workspace& ws = *r.ws;
+    *redo = false;
+    Plan plan;
+    plan_header(r, plan, 1, INT32_MIN);
+    CUDA_TRY(cudaMemsetAsync(ws.hist, 0, sizeof(unsigned) * (size_t)HIST_WORDS, r.st));
+    const unsigned long long range = r.q_end - r.q_begin;
+    const bool direct = r.N <= N_DIRECT_MAX;
+    CUDA_TRY(cudaEventRecord(ws.ev[2], r.st));
+    if (direct) {
+        launch_direct(ws.tab, ws.ctrl, ws.pool, ws.hist, r.N, r.S, (unsigned)range, 1, r.st);
+        LAUNCH_CHECK("direct_kernel");
+        r.stats->kernel_launches += 1;
+        r.stats->enum_launches += 1;
+    } else {
+        // a2': the first X states are formed exactly, one 1024-configuration block per warp -- 2^15 of them without any
+        // threshold, the rest under the threshold those give (which most blocks would pass anyway; X shrinks with S so
+        // that the candidates of this phase, about X S / 2^15, stay far below the pool size). Then walked segments
+        // that double; the last segment takes all the rest and tapers its unit size so that the tail stays short.
+        const unsigned long long prime = 1ull << MIN_CHUNK_BITS;
+        unsigned long long X = 1ull << 21;
+        while (X > prime && X * (unsigned long long)r.S > (1ull << 35)) X >>= 1;
+        if (X > range) X = range;
+        int ns = 0;
+        unsigned long long cur = r.q_begin, units = 0;
+        auto add_segment = [&](unsigned long long sz, int unit_bits, unsigned long long need) {
+            const unsigned long long nu = sz >> unit_bits;
+            plan.seg[ns] = Segment{cur, units, nu, need, unit_bits, 0};
+            units += nu;
+            cur += nu << unit_bits;
+            ++ns;
+        };
+        add_segment(prime, LOWBITS, 0ull);
+        if (X > prime) add_segment(X - prime, LOWBITS, prime);
+        while (cur < r.q_end) {
+            const unsigned long long processed = cur - r.q_begin, remaining = r.q_end - cur;
+            const unsigned long long need = processed / 2 > prime ? processed / 2 : prime;
+            unsigned long long target = (unsigned long long)r.growth * processed;
+            if (ns >= MAX_SEGMENTS - 12) { t_last_error = "internal: bad work plan"; return ISING_ERR_INTERNAL; }
+            if (target < remaining && target < (1ull << r.chunk_log2)) {
+                const int Lw = choose_lw(cur, target, r.lw_max);
+                add_segment(target, MIN_CHUNK_BITS + Lw, need);
+                continue;
+            }
+            // last segment(s): 7/8 of what is left at the full walk length, then 7/8 of the rest with 8x shorter units, ...
+            int Lw = choose_lw(cur, remaining, r.lw_max);
+            while (cur < r.q_end) {
+                const unsigned long long left = r.q_end - cur;
+                while (Lw > 0 && (cur & ((1ull << (MIN_CHUNK_BITS + Lw)) - 1ull))) --Lw;         // alignment of cur
+                unsigned long long sz = left;                                                  // Lw = 0: all of it
+                if (Lw > 0) sz = (left - (left >> 3)) >> (MIN_CHUNK_BITS + Lw) << (MIN_CHUNK_BITS + Lw);
+                if (sz >> (MIN_CHUNK_BITS + Lw)) {
+                    if (ns >= MAX_SEGMENTS) { t_last_error = "internal: bad work plan"; return ISING_ERR_INTERNAL; }
+                    add_segment(sz, MIN_CHUNK_BITS + Lw, need);
+                }
+                Lw = Lw > 3 ? Lw - 3 : 0;
+            }
+        }
+        plan.nseg = ns;
+        plan.total_units = units;
+        int rc = launch_walk(r, plan);
+        if (rc != ISING_OK) return rc;
+    }
+    CUDA_TRY(cudaEventRecord(ws.ev[3], r.st));
+    r.stats->kernel_launches += launch_compact(ws.pool, ws.pool2, ws.ctrl, plan, r.st);
+    LAUNCH_CHECK("compact_kernel");
+    r.stats->kernel_launches += launch_final_small(r.mode ? r.Jorig : r.J, r.mode ? r.horig : r.h, r.N, r.mode, ws.pool2,
+                                                   ws.ctrl, r.S, r.keep_cap, states_out, energies_out, r.st);
+    LAUNCH_CHECK("final_small_kernel");
+    int rc = read_ctrl(r);
+    if (rc != ISING_OK) return rc;
+    float ms = 0.f;
+    CUDA_TRY(cudaEventElapsedTime(&ms, ws.ev[2], ws.ev[3]));
+    r.enum_ms += ms;
+    const Ctrl& c = *ws.h_ctrl;
+    if (c.status != ISING_OK) return ISING_OK;          // rejected by the staging kernel: the caller reports it
+    r.stats->configs += range;
+    if (c.pool_overflow) { *redo = true; return ISING_OK; }
+    r.stats->candidates += c.count;
+    if (c.final_state == 1) { r.stats->keep = (int)c.kept; return ISING_OK; }
+    if (c.final_state != 2 || c.count2 < (unsigned)r.S) {
+        t_last_error = "internal: fewer candidates than requested states";
+        return ISING_ERR_INTERNAL;
+    }
+    // many candidates (large S): the general multi-block selection on the compacted pool
+    r.stats->kernel_launches += launch_select(ws.pool2, ws.ctrl, c.count2, r.S, plan, r.st);
+    LAUNCH_CHECK("select kernels");
+    rc = read_ctrl(r);
+    if (rc != ISING_OK) return rc;
+    if (ws.h_ctrl->band_overflow) {
+        // the kept list was cut: bring the cut list to `pool`, where the band pass expects it
+        copy_entries_kernel<<<(ws.h_ctrl->kept + 255) / 256, 256, 0, r.st>>>(ws.pool2, ws.pool, ws.h_ctrl->kept);
+        LAUNCH_CHECK("copy_entries_kernel");
+        r.stats->kernel_launches += 1;
+        return ISING_OK;
+    }
+    r.stats->keep = (int)ws.h_ctrl->kept;
+    r.stats->kernel_launches += launch_final(r.mode ? r.Jorig : r.J, r.mode ? r.horig : r.h, r.N, r.mode, ws.pool2,
+                                             ws.h_ctrl->kept, r.S, states_out, energies_out, r.st);
+    LAUNCH_CHECK("final kernels");
+    return ISING_OK;
+}
 
 struct Piece {
     unsigned long long base;
-    unsigned nthreads;
-    int Lw;
-    bool direct;                    // the priming piece: one thread per state (direct_kernel)
+    unsigned long long n_units;
+    int unit_bits;
 };
+
+// ---- host-sequenced path: the range in pieces, a selection (normal mode) or an fp64 drain (band mode) after every
+// piece, a piece whose candidates overflow the pool re-run in halves. Used when the single pass was void (adversarial
+// orderings, very large S late in the spectrum) and for the band pass. Leaves the kept list in pool[0..kept). ----
+int run_pieces(Run& r, bool band_mode, int loE, unsigned want)
+{
+    Workspace& ws = *r.ws;
+    Plan plan;
+    plan_header(r, plan, 0, band_mode ? loE : INT32_MIN);
+    plan.nseg = 1;
+    unsigned long long cur = r.q_begin, processed = 0;
+    std::vector<Piece> stack;
+    bool tau_finite = band_mode;
+    while (cur < r.q_end || !stack.empty()) {
+        Piece pc;
+        if (!stack.empty()) {
+            pc = stack.back();
+            stack.pop_back();
+        } else if (r.N <= N_DIRECT_MAX) {
+            pc = Piece{cur, (r.q_end - cur) >> (r.N < LOWBITS ? r.N : LOWBITS), r.N < LOWBITS ? r.N : LOWBITS};
+            cur = r.q_end;
+        } else if (processed == 0 && !band_mode) {
+            pc = Piece{cur, 1ull << (MIN_CHUNK_BITS - LOWBITS), LOWBITS};      // a2': formed exactly
+            cur += 1ull << MIN_CHUNK_BITS;
+        } else {
+            const unsigned long long remaining = r.q_end - cur;
+            unsigned long long target = band_mode ? (1ull << r.chunk_log2) : (unsigned long long)r.growth * 3ull * processed;
+            if (target > (1ull << r.chunk_log2)) target = 1ull << r.chunk_log2;
+            if (!tau_finite && target > (1ull << 16)) target = 1ull << 16;     // everything passes: keep it small
+            if (target < (1ull << MIN_CHUNK_BITS)) target = 1ull << MIN_CHUNK_BITS;
+            const unsigned long long sz = target < remaining ? target : remaining;
+            const int Lw = choose_lw(cur, sz, r.lw_max);
+            pc = Piece{cur, sz >> (MIN_CHUNK_BITS + Lw), MIN_CHUNK_BITS + Lw};
+            if (pc.n_units == 0) { t_last_error = "internal: bad launch plan"; return ISING_ERR_INTERNAL; }
+            cur += pc.n_units << pc.unit_bits;
+        }
+        const unsigned long long pc_size = pc.n_units << pc.unit_bits;
+        if (r.N <= N_DIRECT_MAX) {
+            // tiny instance: everything at once through the direct kernel (its 2^N states always fit)
+            launch_direct(ws.tab, ws.ctrl, ws.pool, ws.hist, r.N, r.S, (unsigned)(r.q_end - r.q_begin), 0, r.st);
+            LAUNCH_CHECK("direct_kernel");
+            r.stats->kernel_launches += 1;
+            r.stats->enum_launches += 1;
+        } else {
+            plan.seg[0] = Segment{pc.base, 0ull, pc.n_units, 0ull, pc.unit_bits, 0};
+            plan.total_units = pc.n_units;
+            plan.q_end = r.q_end;
+            reset_queue_kernel<<<1, 1, 0, r.st>>>(ws.ctrl, 0);
+            CUDA_TRY(cudaEventRecord(ws.ev[2], r.st));
+            int rc = launch_walk(r, plan);
+            if (rc != ISING_OK) return rc;
+            CUDA_TRY(cudaEventRecord(ws.ev[3], r.st));
+            r.stats->kernel_launches += 1;
+        }
+        int rc = read_ctrl(r);
+        if (rc != ISING_OK) return rc;
+        if (r.N > N_DIRECT_MAX) {
+            float ms = 0.f;
+            CUDA_TRY(cudaEventElapsedTime(&ms, ws.ev[2], ws.ev[3]));
+            r.enum_ms += ms;
+        }
+        const unsigned count = ws.h_ctrl->count, kept = ws.h_ctrl->kept;
+        if (ws.h_ctrl->pool_overflow) {
+            // pool overflow: drop this piece's candidates and run it again in two halves
+            reset_queue_kernel<<<1, 1, 0, r.st>>>(ws.ctrl, 1);
+            r.stats->kernel_launches += 1;
+            r.stats->split_retries += 1;
+            Piece a = pc, b = pc;
+            if (pc.n_units >= 2) {
+                a.n_units = pc.n_units / 2;
+                b.n_units = pc.n_units - a.n_units;
+                b.base = pc.base + (a.n_units << pc.unit_bits);
+            } else if (pc.unit_bits > MIN_CHUNK_BITS) {
+                a.unit_bits = b.unit_bits = pc.unit_bits - 1;
+                a.n_units = b.n_units = 1;
+                b.base = pc.base + (1ull << a.unit_bits);
+            } else {
+                t_last_error = "internal: candidate pool overflow on a minimal launch";
+                return ISING_ERR_INTERNAL;
+            }
+            stack.push_back(b);
+            stack.push_back(a);
+            continue;
+        }
+        processed += pc_size;
+        r.stats->configs += pc_size;
+        r.stats->candidates += count - kept;
+        if (band_mode) {
+            if (count > kept)
+                r.stats->kernel_launches += launch_band_drain(r.mode ? r.Jorig : r.J, r.mode ? r.horig : r.h, r.N, r.mode,
+                                                              ws.pool, ws.ctrl, kept, count, want, r.st);
+        } else if (count > kept) {
+            r.stats->kernel_launches += launch_select(ws.pool, ws.ctrl, count, r.S, plan, r.st);
+            if (count >= (unsigned)r.S) tau_finite = true;
+        }
+        LAUNCH_CHECK("selection kernels");
+    }
+    return read_ctrl(r);
+}
 
 // mode 0: (J, h) is an Ising instance, energies by eq. (1). mode 1: (Jorig, horig) = QUBO (a, b); (J, h) its Ising image.
 int run_lowest(const double* J, const double* h, const double* Jorig, const double* horig, int mode, double extra_eps_rel,
@@ -102,16 +428,39 @@ int run_lowest(const double* J, const double* h, const double* Jorig, const doub
     Workspace& ws = t_ws;
     ising_stats stats;
     memset(&stats, 0, sizeof(stats));
-    const int lw_run = env_int("ISING_LW", LW_MAX, 0, LW_MAX);
-    const int chunk_log2 = env_int("ISING_CHUNK_LOG2", 42, MIN_CHUNK_BITS, 44);
-    const int growth = env_int("ISING_GROWTH", 3, 1, 1 << 20);   // a launch is at most growth x what has been processed
-    const int variant = env_int("ISING_KERNEL", 16, 16, 32) == 32 ? 32 : 16;   // 16: packed screen, 32: int32 kernel
+    Run r;
+    r.ws = &ws; r.stats = &stats;
+    r.J = J; r.h = h; r.Jorig = Jorig; r.horig = horig;
+    r.mode = mode; r.N = N; r.S = S;
+    r.lw_max = env_int("ISING_LW", LW_MAX, 0, LW_MAX);
+    r.chunk_log2 = env_int("ISING_CHUNK_LOG2", 42, MIN_CHUNK_BITS, 44);
+    r.growth = env_int("ISING_GROWTH", 1, 1, 1 << 20);      // a segment is at most growth x what lies before it
+    r.variant = env_int("ISING_KERNEL", 16, 16, 32) == 32 ? 32 : 16;   // 16: packed screen, 32: int32 kernel
+    // test knob for the band pass: a selection keeps at most 2^k entries (never fewer than S)
+    r.keep_cap = 1u << env_int("ISING_KEEP_CAP_LOG2", 20, 5, 20);
+    while (r.keep_cap < (unsigned)S) r.keep_cap <<= 1;
+    const int path = env_int("ISING_PATH", 0, 0, 1);        // 1: skip the single pass (tests of the host-sequenced path)
+    r.q_begin = q_begin; r.q_end = q_end; r.st = st; r.enum_ms = 0.0;
+    const int rb = floor_log2(q_end - q_begin - 1) + 1;     // bits of the range
+    r.qshift = rb > 31 ? rb - 31 : 0;                       // (range >> qshift) < 2^32 - 1
 
     CUDA_TRY(cudaEventRecord(ws.ev[0], st));
     launch_stage(J, h, N, ws.tab, ws.ctrl, st, extra_eps_rel);
+    LAUNCH_CHECK("stage kernels");
     stats.kernel_launches += 2;
-    CUDA_TRY(cudaMemcpyAsync(ws.h_ctrl, ws.ctrl, sizeof(Ctrl), cudaMemcpyDeviceToHost, st));
-    CUDA_TRY(cudaStreamSynchronize(st));
+    stats.inner_bits = LOWBITS;
+    stats.kernel_variant = r.variant;
+    stats.passes = 1;
+
+    bool redo = (path == 1);
+    int rc = ISING_OK;
+    if (!redo) {
+        rc = run_single_pass(r, states_out, energies_out, &redo);
+        if (rc != ISING_OK) return rc;
+    } else {
+        rc = read_ctrl(r);
+        if (rc != ISING_OK) return rc;
+    }
     if (ws.h_ctrl->status != ISING_OK) {
         t_last_error = std::string("instance rejected: ") + ising_strerror(ws.h_ctrl->status);
         return ws.h_ctrl->status;
@@ -119,119 +468,67 @@ int run_lowest(const double* J, const double* h, const double* Jorig, const doub
     stats.grid_exponent = ws.h_ctrl->p;
     stats.exact = ws.h_ctrl->exact;
     stats.epsilon = ws.h_ctrl->epsilon;
-    stats.inner_bits = LOWBITS;
-    stats.kernel_variant = variant;
-    stats.screen_shift = variant == 16 ? ws.h_ctrl->shift16 : -1;
-    stats.passes = 1;
+    stats.screen_shift = r.variant == 16 ? ws.h_ctrl->shift16 : -1;
+    const int band = ws.h_ctrl->band;
 
-    double enum_ms = 0.0;
-    unsigned kept = 0;
-    if (N <= N_DIRECT_MAX) {
-        launch_direct(ws.tab, ws.ctrl, ws.pool, N, 0, 1u << N, 0, st);
+    if (redo) {
+        // the single pass was void (or skipped): the same range again, host-sequenced
+        if (path == 0) { stats.passes += 1; stats.configs = 0; stats.candidates = 0; }
+        restart_kernel<<<1, 1, 0, st>>>(ws.ctrl, tau_pack(TAU_INF, QC_NONE));
+        LAUNCH_CHECK("restart_kernel");
         stats.kernel_launches += 1;
-        stats.enum_launches += 1;
-        stats.configs = 1ull << N;
-        stats.candidates = 1ull << N;
-        stats.kernel_launches += launch_select(ws.pool, ws.ctrl, 1u << N, S, st);
-    } else {
-        unsigned long long cur = q_begin, processed = 0;
-        std::vector<Piece> stack;
-        bool tau_finite = false;
-        while (cur < q_end || !stack.empty()) {
-            Piece pc;
-            if (!stack.empty()) {
-                pc = stack.back();
-                stack.pop_back();
-            } else {
-                const unsigned long long remaining = q_end - cur;
-                unsigned long long target = 1ull << MIN_CHUNK_BITS;
-                if (processed > 0) {
-                    target = (unsigned long long)growth * processed;
-                    if (target > (1ull << chunk_log2)) target = 1ull << chunk_log2;
-                    if (!tau_finite && target > (1ull << 16)) target = 1ull << 16;   // everything passes: keep it small
-                }
-                const unsigned long long sz = target < remaining ? target : remaining;
-                int Lw = floor_log2(sz) - 27;
-                Lw = Lw < 0 ? 0 : (Lw > lw_run ? lw_run : Lw);
-                while (Lw > 0 && (cur & ((1ull << (LOWBITS + Lw)) - 1))) --Lw;
-                unsigned long long nt = (sz >> (LOWBITS + Lw)) / 32 * 32;
-                if (nt < 32 || nt > 0x7fffffe0ull) {
-                    t_last_error = "internal: bad launch plan";
-                    return ISING_ERR_INTERNAL;
-                }
-                pc.base = cur;
-                pc.nthreads = (unsigned)nt;
-                pc.Lw = Lw;
-                pc.direct = (processed == 0);          // a2': the first 2^15 states, tau = +inf
-                cur += nt << (LOWBITS + Lw);
-            }
-            CUDA_TRY(cudaEventRecord(ws.ev[2], st));
-            if (pc.direct) launch_direct(ws.tab, ws.ctrl, ws.pool, N, pc.base, pc.nthreads << (LOWBITS + pc.Lw), 0, st);
-            else if (variant == 16) launch_enumerate16(ws.tab, ws.ctrl, ws.pool, N, pc.Lw, pc.base, pc.nthreads,
-                                                       processed < (1ull << 30), st);
-            else launch_enumerate(ws.tab, ws.ctrl, ws.pool, N, pc.Lw, pc.base, pc.nthreads, st);
-            CUDA_TRY(cudaEventRecord(ws.ev[3], st));
-            stats.kernel_launches += 1;
-            stats.enum_launches += 1;
-            CUDA_TRY(cudaMemcpyAsync(ws.h_ctrl, ws.ctrl, sizeof(Ctrl), cudaMemcpyDeviceToHost, st));
-            CUDA_TRY(cudaStreamSynchronize(st));
-            float ms = 0.f;
-            CUDA_TRY(cudaEventElapsedTime(&ms, ws.ev[2], ws.ev[3]));
-            enum_ms += ms;
-            const unsigned count = ws.h_ctrl->count;
-            kept = ws.h_ctrl->kept;
-            const unsigned long long pc_size = (unsigned long long)pc.nthreads << (LOWBITS + pc.Lw);
-            if (count > POOL_CAP) {
-                // pool overflow: drop this piece's candidates and run it again in two halves
-                reset_count_kernel<<<1, 1, 0, st>>>(ws.ctrl);
-                stats.kernel_launches += 1;
-                stats.split_retries += 1;
-                Piece a = pc, b = pc;
-                a.direct = b.direct = false;
-                if (pc.nthreads >= 64) {
-                    a.nthreads = pc.nthreads / 64 * 32;
-                    b.nthreads = pc.nthreads - a.nthreads;
-                    b.base = pc.base + ((unsigned long long)a.nthreads << (LOWBITS + pc.Lw));
-                } else if (pc.Lw > 0) {
-                    a.Lw = b.Lw = pc.Lw - 1;
-                    b.base = pc.base + (32ull << (LOWBITS + a.Lw));
-                } else {
-                    t_last_error = "internal: candidate pool overflow on a minimal launch";
-                    return ISING_ERR_INTERNAL;
-                }
-                stack.push_back(b);
-                stack.push_back(a);
-                continue;
-            }
-            processed += pc_size;
-            stats.configs += pc_size;
-            stats.candidates += count - kept;
-            if (count > kept) {
-                stats.kernel_launches += launch_select(ws.pool, ws.ctrl, count, S, st);
-                if (count >= (unsigned)S) tau_finite = true;
-            }
+        rc = run_pieces(r, false, 0, 0);
+        if (rc != ISING_OK) return rc;
+        if (!ws.h_ctrl->band_overflow) {
+            const unsigned kept = ws.h_ctrl->kept;
+            if (kept < (unsigned)S) { t_last_error = "internal: fewer states kept than requested"; return ISING_ERR_INTERNAL; }
+            stats.keep = (int)kept;
+            stats.kernel_launches += launch_final(mode ? Jorig : J, mode ? horig : h, N, mode, ws.pool, kept, S,
+                                                  states_out, energies_out, st);
+            LAUNCH_CHECK("final kernels");
         }
     }
-    CUDA_TRY(cudaMemcpyAsync(ws.h_ctrl, ws.ctrl, sizeof(Ctrl), cudaMemcpyDeviceToHost, st));
-    CUDA_TRY(cudaStreamSynchronize(st));
     if (ws.h_ctrl->band_overflow) {
-        t_last_error = "guard band holds more than KEEP_CAP states; the S-th level cannot be certified";
-        return ISING_ERR_BAND;
+        // ---- G3 fallback: more than KEEP_CAP states lie within the guard band of the S-th
+        // lowest grid energy eS, so the band cannot be kept resident. Every state with grid energy < eS - band is
+        // certainly among the S lowest (they are a sorted prefix of the kept list); the others come from the states
+        // with grid energy in [eS - band, eS + band], which a second enumeration streams through the pool: each
+        // piece's band states are re-evaluated in fp64 and merged into the running best S - n_sure under (E64, q).
+        const unsigned kept = ws.h_ctrl->kept;
+        const int eS = ws.h_ctrl->eS;
+        count_sure_kernel<<<1, 32, 0, st>>>(ws.pool, ws.ctrl, kept, band);
+        LAUNCH_CHECK("count_sure_kernel");
+        rc = read_ctrl(r);
+        if (rc != ISING_OK) return rc;
+        const unsigned n_sure = ws.h_ctrl->n_sure;
+        if (n_sure >= (unsigned)S) { t_last_error = "internal: band pass bookkeeping"; return ISING_ERR_INTERNAL; }
+        if (n_sure) {
+            copy_entries_kernel<<<(n_sure + 255) / 256, 256, 0, st>>>(ws.pool, ws.pool2, n_sure);
+            LAUNCH_CHECK("copy_entries_kernel");
+        }
+        const long long hi = (long long)eS + band;
+        restart_kernel<<<1, 1, 0, st>>>(ws.ctrl, tau_pack(hi < (long long)TAU_INF ? (int)hi : TAU_INF, QC_NONE));
+        LAUNCH_CHECK("restart_kernel");
+        stats.kernel_launches += 3;
+        stats.passes += 1;
+        const unsigned want = (unsigned)S - n_sure;
+        rc = run_pieces(r, true, eS - band, want);
+        if (rc != ISING_OK) return rc;
+        if (ws.h_ctrl->kept < want) { t_last_error = "internal: band pass found too few states"; return ISING_ERR_INTERNAL; }
+        // final list = sure states + best band states: pool2[0..n_sure) + pool[0..want), all re-evaluated in fp64
+        copy_entries_kernel<<<(want + 255) / 256, 256, 0, st>>>(ws.pool, ws.pool2 + n_sure, want);
+        LAUNCH_CHECK("copy_entries_kernel");
+        stats.keep = S;
+        stats.kernel_launches += 1 + launch_final(mode ? Jorig : J, mode ? horig : h, N, mode, ws.pool2, (unsigned)S, S,
+                                                  states_out, energies_out, st);
+        LAUNCH_CHECK("final kernels");
     }
-    kept = ws.h_ctrl->kept;
-    if (kept < (unsigned)S) {
-        t_last_error = "internal: fewer states kept than requested";
-        return ISING_ERR_INTERNAL;
-    }
-    stats.keep = (int)kept;
-    stats.kernel_launches += launch_final(mode ? Jorig : J, mode ? horig : h, N, mode, ws.pool, kept, S,
-                                          states_out, energies_out, st);
     CUDA_TRY(cudaEventRecord(ws.ev[1], st));
     CUDA_TRY(cudaStreamSynchronize(st));
     CUDA_TRY(cudaGetLastError());
     float total_ms = 0.f;
     CUDA_TRY(cudaEventElapsedTime(&total_ms, ws.ev[0], ws.ev[1]));
-    stats.enum_ms = enum_ms;
+    stats.enum_ms = r.enum_ms;
     stats.total_ms = total_ms;
     t_stats = stats;
     t_have_stats = true;
@@ -556,6 +853,15 @@ int ising_addmin16x2_peak(double ms_target, double* inst_per_s_out_host, void* s
     return ISING_OK;
 }
 
-void ising_release_workspace(void) { t_ws.release(); }
+int ising_addmin_mix_peak(double ms_target, double* addmin_per_s_out_host, void* stream)
+{
+    if (!addmin_per_s_out_host) return ISING_ERR_NULL;
+    double r = run_fma_peak(ms_target, (cudaStream_t)stream, 3);
+    if (r < 0.0) { t_last_error = "add-min mix microbenchmark failed"; return ISING_ERR_CUDA; }
+    *addmin_per_s_out_host = r;
+    return ISING_OK;
+}
+
+void ising_release_workspace(void) { if (t_ws.device >= 0) t_ws.release(); }
 
 }  // extern "C"

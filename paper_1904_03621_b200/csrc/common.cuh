@@ -5,8 +5,13 @@
 //   L  = "lo"   spins 0..LL-1          : per-thread register table V[2^LL]
 //   M  = "mid"  spins LL..LL+LM-1      : per-thread register table U[2^LM], shared table C[2^LM][2^LL]
 //   W  = "walk" spins LL+LM..+Lw-1     : walked by every thread in reflected Gray order
-//   T  = "thread" spins above          : lane, warp, block and launch-base bits; fixed per thread
+//   T  = "thread" spins above          : lane bits and the bits of the work unit; fixed per thread
 //   all energies in the kernels are int32 multiples of the grid 2^-p (stage.cu chooses p).
+//
+// Work distribution: the state range of a call is cut into SEGMENTS of geometrically
+// growing size; a segment is cut into equal UNITS (one warp each: 32 lanes x 2^Lw Gray steps x 1024 configurations,
+// or, for the very first segment, one 1024-configuration block formed exactly). The persistent enumeration kernel
+// hands units out in ascending order of q through an atomic counter in Ctrl.
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
@@ -25,11 +30,24 @@ constexpr int WQ_BITS = 27;              // sum|Jq| + sum|hq| <= 2^27 grid units
 constexpr int TAU_INF = 0x3fffffff;      // "no threshold yet"; every grid energy is far below it
 constexpr unsigned long long Q_MAX = ~0ull;
 
-constexpr unsigned POOL_CAP_LOG2 = 21;
-constexpr unsigned POOL_CAP = 1u << POOL_CAP_LOG2;     // entries in the candidate pool
+// Sign convention of the field term (reading G2): +1 implements eq. (1) AS PRINTED, H = -sum J s s - sum h s
+// (PAPER.md:43), whose fields-only ground state is s_i = +sign(h_i). The other reading some texts use,
+// H' = -sum J s s + sum h s = H(J, -h), is this constant set to -1: it is applied wherever h enters the library --
+// the quantised fields hq (stage.cu), the fp64 re-evaluation (select.cu) and the QUBO conversion (stage.cu).
+constexpr double FIELD_TERM_SIGN = 1.0;
+
+constexpr unsigned POOL_CAP_LOG2 = 22;
+constexpr unsigned POOL_CAP = 1u << POOL_CAP_LOG2;     // entries in each of the two candidate pools (64 MiB each)
 constexpr unsigned KEEP_CAP = 1u << 20;                // most entries kept after a selection
 constexpr int SORT_TILE = 4096;                        // entries sorted by one block in shared memory
 constexpr int SORT_THREADS = 1024;
+
+constexpr int HIST_COARSE = 256;                       // coarse bins: 256 fine bins each
+constexpr int HIST_FINE = 65536;                       // fine bins over [-Wq, +Wq]
+constexpr int HIST_WORDS = HIST_COARSE + HIST_FINE;    // hist[0..256) coarse, hist[256..) fine
+constexpr int MAX_SEGMENTS = 64;
+constexpr int WALK_THREADS = 256;                      // threads per block of the enumeration kernels
+constexpr int WALK_WARPS = WALK_THREADS / 32;
 
 // One candidate: sortable 64-bit key (grid energy or fp64 energy, order preserving) and the state index.
 struct __align__(16) Entry {
@@ -61,6 +79,17 @@ __device__ inline double f64_from_key(unsigned long long k)
     return __longlong_as_double((long long)b);
 }
 
+// The filter threshold is ONE 64-bit word so that it can be published with a single atomicMin and read with a single
+// load:  tau = key32(tauE) << 32 | Qc.   A configuration (e, q) passes iff  e < tauE  or  (e == tauE and q < tauQ),
+// tauQ = q_begin + (Qc << qshift), Qc = 0xffffffff meaning "no limit on q". A SMALLER word is a TIGHTER threshold.
+constexpr unsigned QC_NONE = 0xffffffffu;
+__host__ __device__ inline unsigned long long tau_pack(int tauE, unsigned qc)
+{
+    return (key_from_i32(tauE) << 32) | (unsigned long long)qc;
+}
+__host__ __device__ inline int tau_energy(unsigned long long tau) { return i32_from_key(tau >> 32); }
+__host__ __device__ inline unsigned tau_qc(unsigned long long tau) { return (unsigned)tau; }
+
 // Device-resident control block of one call; the host reads it back through pinned memory.
 struct Ctrl {
     int status;            // ISING_OK or an ISING_ERR_* found by the staging kernel
@@ -69,14 +98,24 @@ struct Ctrl {
     int band;              // guard band in grid units: candidates are kept up to E_S + band
     double epsilon;        // bound on |grid energy * 2^-p - eq.(1) energy|
     double W;              // sum_{i<j}|J_ij| + sum_i|h_i|
-    unsigned count;        // entries in the pool (kept prefix + new candidates); may exceed POOL_CAP = overflow
+    long long Wq;          // sum_{i<j}|Jq_ij| + sum_i|hq_i|: every grid energy lies in [-Wq, +Wq]
+    unsigned count;        // entries in the pool (kept prefix + new candidates); pushes beyond POOL_CAP are dropped
     unsigned kept;         // entries of the sorted prefix after the last selection
-    int tauE;              // filter threshold (grid units)
+    unsigned long long tau;        // filter threshold word (tau_pack)
     int shift16;           // copy of Tables::shift16 (written by tables_kernel) for the host's statistics
-    unsigned long long tauQ;   // ties on tauE pass only for q < tauQ
-    unsigned band_overflow;    // selection wanted to keep more than KEEP_CAP entries
-    unsigned pad1;
-    unsigned long long candidates;   // running total of pushes
+    int hist_shift;        // histogram bin of grid energy e:  (e + Wq) >> hist_shift   (fine bin, < HIST_FINE)
+    unsigned band_overflow;    // selection wanted to keep more than KEEP_CAP entries (sticky)
+    unsigned pool_overflow;    // a push did not fit into the pool (sticky): the run is void and is redone piecewise
+    unsigned long long next_unit;      // work queue: next unit to hand out
+    unsigned long long done_configs;   // configurations of completed units (ramp-up rule, see Segment::need_done)
+    unsigned count2;           // entries of the compacted pool
+    unsigned final_state;      // written by final_small_kernel: 0 not run, 1 done, 2 too many entries for one block
+    int eS;                    // S-th smallest grid energy at the final selection (for the band pass)
+    unsigned n_sure;           // band pass: entries below the band (certainly among the S lowest)
+    unsigned blocks_done;      // direct kernel: blocks that have finished (the last one derives the threshold)
+    unsigned pad0;
+    unsigned long long hits;   // 1024-configuration blocks that passed the screen and were formed exactly
+    unsigned long long false_hits;     // ... of which none passed the exact test
 };
 
 // Instance tables in grid units, built once per call by build_tables (stage.cu).
@@ -100,26 +139,47 @@ struct Tables {
     unsigned DUp[LW_MAX * 2 * (NMID / 2)]; // DUp[k][sb][u]  = +-((DU[k][1][m0] >> s) + 65536 (DU[k][1][m0 | 8] >> s))
 };
 
-struct Geometry {
+// One segment of the work plan: n_units units of 2^unit_bits configurations starting at state q0.
+struct Segment {
+    unsigned long long q0;
+    unsigned long long first_unit;     // index of the segment's first unit in the queue
+    unsigned long long n_units;
+    unsigned long long need_done;      // a unit of this segment starts only after this many configurations are done:
+                                       // the threshold is then good enough for most blocks to fail the screen
+    int unit_bits;                     // 10: one exactly formed 1024-configuration block; 15 + Lw: a walked unit
+    int pad;
+};
+
+// The work plan of one launch of the enumeration kernel (a kernel parameter: lives in the constant bank).
+struct Plan {
+    Segment seg[MAX_SEGMENTS];
+    unsigned long long total_units;
+    unsigned long long q_begin;        // first state of the CALL (origin of the coarse tie limit Qc)
+    unsigned long long q_end;          // one past the last state this launch enumerates
+    int nseg;
     int N;
-    int Lw;                        // walk bits of this launch
-    unsigned long long base;       // first state of the launch (aligned to the launch size)
+    int S;
+    int use_hist;                      // 1: pushes feed the histogram and the kernel refreshes tau itself
+    int refresh;                       // refresh tau whenever the pool count crosses a multiple of this
+    int qshift;                        // tauQ = q_begin + (Qc << qshift)
+    int loE;                           // band pass: only configurations with grid energy >= loE are pushed
+    unsigned keep_cap;                 // most entries a selection keeps (KEEP_CAP; smaller only in tests of the band pass)
 };
 
 // stage.cu
 void launch_stage(const double* J, const double* h, int N, Tables* tab, Ctrl* ctrl, cudaStream_t st,
                   double extra_eps_rel);
 void launch_qubo_to_ising(const double* a, const double* b, int N, double* J, double* h, cudaStream_t st);
-// enumerate.cu
-void launch_enumerate(const Tables* tab, Ctrl* ctrl, Entry* pool, int N, int Lw,
-                      unsigned long long base, unsigned nthreads, cudaStream_t st);
-void launch_direct(const Tables* tab, Ctrl* ctrl, Entry* pool, int N, unsigned long long base, unsigned count,
-                   unsigned kept, cudaStream_t st);
-// enumerate16.cu
-void launch_enumerate16(const Tables* tab, Ctrl* ctrl, Entry* pool, int N, int Lw,
-                        unsigned long long base, unsigned nthreads, bool heavy_hits, cudaStream_t st);
+// enumerate.cu / enumerate16.cu: the persistent enumeration kernel, int32 and packed 16-bit variants
+void launch_walk32(const Tables* tab, Ctrl* ctrl, Entry* pool, unsigned* hist, const Plan& plan, cudaStream_t st);
+void launch_walk16(const Tables* tab, Ctrl* ctrl, Entry* pool, unsigned* hist, const Plan& plan, cudaStream_t st);
+void launch_direct(const Tables* tab, Ctrl* ctrl, Entry* pool, unsigned* hist, int N, int S, unsigned count,
+                   int use_hist, cudaStream_t st);
 // select.cu
-int  launch_select(Entry* pool, Ctrl* ctrl, unsigned n, int S, cudaStream_t st);     // returns kernels launched
+int  launch_select(Entry* pool, Ctrl* ctrl, unsigned n, int S, const Plan& plan, cudaStream_t st);   // returns kernels launched
+int  launch_compact(const Entry* pool, Entry* pool2, Ctrl* ctrl, const Plan& plan, cudaStream_t st);
+int  launch_final_small(const double* J, const double* h, int N, int mode, Entry* pool2, Ctrl* ctrl, int S,
+                        unsigned keep_cap, unsigned long long* states_out, double* energies_out, cudaStream_t st);
 int  launch_final(const double* J, const double* h, int N, int mode, Entry* pool, unsigned m, int S,
                   unsigned long long* states_out, double* energies_out, cudaStream_t st);
 void launch_energies(const double* J, const double* h, int N, int mode, const unsigned long long* states,
@@ -131,6 +191,9 @@ int  launch_expand_complements(const unsigned long long* states, const double* e
 int  launch_alg1_chunk(const double* J, const double* h, int N, unsigned long long base, unsigned count,
                        Entry* pool, unsigned kept, cudaStream_t st);
 int  launch_emit(const Entry* pool, int S, unsigned long long* states_out, double* energies_out, cudaStream_t st);
+int  launch_band_drain(const double* J, const double* h, int N, int mode, Entry* pool, Ctrl* ctrl, unsigned kept,
+                       unsigned n, unsigned want, cudaStream_t st);
+void set_select_attributes();
 // dos.cu
 void launch_dos(const Tables* tab, int N, int Lw, unsigned long long base, unsigned nthreads, int e_lo, int bshift,
                 int nbins, unsigned long long* hist, cudaStream_t st);

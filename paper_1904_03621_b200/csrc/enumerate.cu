@@ -1,4 +1,5 @@
-// enumerate.cu -- SURVEY.md section 8 rows a2 (thread base state), a3 (enumeration) and a4 (threshold filter).
+// enumerate.cu -- SURVEY.md section 8 rows a2 (base state), a3 (enumeration) and a4 (threshold filter), int32 variant,
+// and the direct kernel for tiny instances.
 //
 // Every configuration's grid energy is formed exactly once, as   E = Eh + U[mid] + (V[lo] + C[mid][lo]),
 // the QUBO decomposition of eqs. (2),(3) around the thread's base state q0:
@@ -15,173 +16,107 @@
 // Walk (north_star (a), Gray code): the thread's Lw walk bits advance in reflected Gray order; flipping walk bit k
 // adds a warp-uniform row DV[k][.] to V, DU[k][.] to U, and DW[t] -+ 2 Phi_k to Eh (the O(N) local-field
 // update of the classic Gray walk, restricted to the 64 table entries that depend on bit k).
-#include "common.cuh"
+//
+// This is the arithmetic "no narrower than the paper's" (32-bit, exact): the default kernel (enumerate16.cu) screens
+// in 16 bits and reaches the same candidate set. Selected with ISING_KERNEL=32; work distribution, base state and
+// the exact forming of hit blocks are shared with it (walk.cuh).
+#include "walk.cuh"
 
 namespace ising {
 
-__device__ __forceinline__ void push_candidate(Ctrl* ctrl, Entry* pool, int e, unsigned long long q)
-{
-    unsigned idx = atomicAdd(&ctrl->count, 1u);
-    if (idx < POOL_CAP) {
-        Entry en;
-        en.key = key_from_i32(e);
-        en.q = q;
-        pool[idx] = en;
+struct Inner32 {
+    struct Shared {
+        __align__(16) int C[NMID * NLO];
+        __align__(16) int DV[LW_MAX * 2 * NLO];
+        __align__(16) int DU[LW_MAX * 2 * NMID];
+    };
+    struct Regs {
+        int V[NLO], U[NMID];
+    };
+
+    static __device__ __forceinline__ void load_shared(Shared& sh, const Tables* __restrict__ tab)
+    {
+        for (int i = threadIdx.x; i < NMID * NLO; i += blockDim.x) sh.C[i] = tab->C[i];
+        for (int i = threadIdx.x; i < LW_MAX * 2 * NLO; i += blockDim.x) sh.DV[i] = tab->DV[i];
+        for (int i = threadIdx.x; i < LW_MAX * 2 * NMID; i += blockDim.x) sh.DU[i] = tab->DU[i];
     }
-}
 
-constexpr int ENUM_THREADS = 256;
-
-__global__ void __launch_bounds__(ENUM_THREADS, 2)
-enumerate_kernel(const Tables* __restrict__ tab, Ctrl* __restrict__ ctrl, Entry* __restrict__ pool,
-                 int N, int Lw, unsigned long long base, unsigned nthreads)
-{
-    __shared__ __align__(16) int sC[NMID * NLO];
-    __shared__ __align__(16) int sDV[LW_MAX * 2 * NLO];
-    __shared__ __align__(16) int sDU[LW_MAX * 2 * NMID];
-    __shared__ int sDW[1 << LW_MAX];
-    __shared__ int sScratch[ENUM_THREADS / 32][NLO + NMID];
-
-    for (int i = threadIdx.x; i < NMID * NLO; i += blockDim.x) sC[i] = tab->C[i];
-    for (int i = threadIdx.x; i < LW_MAX * 2 * NLO; i += blockDim.x) sDV[i] = tab->DV[i];
-    for (int i = threadIdx.x; i < LW_MAX * 2 * NMID; i += blockDim.x) sDU[i] = tab->DU[i];
-    for (int i = threadIdx.x; i < (1 << Lw); i += blockDim.x) sDW[i] = tab->DW[i];
-    __syncthreads();
-
-    const unsigned gtid = blockIdx.x * blockDim.x + threadIdx.x;
-    if (gtid >= nthreads) return;                  // nthreads is a multiple of 32: whole warps leave together
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int nlow = LOWBITS + Lw;
-    const unsigned long long q0 = base + ((unsigned long long)gtid << nlow);
-
-    // ---- a2: base state. E0 = E(q0) by eq. (1); Phi_i(q0) = hq_i + sum_j Jq_ij s_j(q0) for the L, M, W spins ----
-    const int* __restrict__ Jq = tab->Jq;
-    const int* __restrict__ hq = tab->hq;
-    int E0 = 0;
-    for (int i = 0; i < N; ++i) {
-        const unsigned bi = (unsigned)(q0 >> i) & 1u;
-        const int* row = Jq + i * 64;
-        int acc = 0;
-        for (int j = i + 1; j < N; ++j) {
-            const unsigned bj = (unsigned)(q0 >> j) & 1u;
-            const int v = row[j];
-            acc += (bi ^ bj) ? v : -v;             // -J s_i s_j
+    static __device__ __forceinline__ void init(Regs& R, const Tables* __restrict__ tab, const int (&Phi)[LOWBITS])
+    {
+#pragma unroll
+        for (int x = 0; x < NLO; ++x) {
+            int a = tab->QL[x];
+#pragma unroll
+            for (int i = 0; i < LL; ++i) if (x >> i & 1) a -= 2 * Phi[i];
+            R.V[x] = a;
         }
-        const int hv = hq[i];
-        E0 += acc + (bi ? -hv : hv);               // -h s_i
-    }
-    int Phi[LOWBITS];
-    int PhiW[LW_MAX];
 #pragma unroll
-    for (int i = 0; i < LOWBITS + LW_MAX; ++i) {
-        int acc = 0;
-        if (i < nlow && i < N) {
-            const int* row = Jq + i * 64;
-            acc = hq[i];
-            for (int j = 0; j < N; ++j) {
-                const int v = row[j];              // Jq_ii = 0
-                acc += ((unsigned)(q0 >> j) & 1u) ? v : -v;
-            }
+        for (int x = 0; x < NMID; ++x) {
+            int a = tab->QM[x];
+#pragma unroll
+            for (int j = 0; j < LM; ++j) if (x >> j & 1) a -= 2 * Phi[LL + j];
+            R.U[x] = a;
         }
-        if (i < LOWBITS) Phi[i] = acc; else PhiW[i - LOWBITS] = acc;
     }
-    int V[NLO], U[NMID];
-#pragma unroll
-    for (int x = 0; x < NLO; ++x) {
-        int a = tab->QL[x];
-#pragma unroll
-        for (int i = 0; i < LL; ++i) if (x >> i & 1) a -= 2 * Phi[i];
-        V[x] = a;
-    }
-#pragma unroll
-    for (int x = 0; x < NMID; ++x) {
-        int a = tab->QM[x];
-#pragma unroll
-        for (int j = 0; j < LM; ++j) if (x >> j & 1) a -= 2 * Phi[LL + j];
-        U[x] = a;
-    }
-    int Eh = E0;
 
-    const int tauE = ctrl->tauE;
-    const unsigned long long tauQ = ctrl->tauQ;
-    int* scratch = sScratch[warp];
-    const unsigned long long q0_warp = q0 - ((unsigned long long)lane << nlow);
-
-    const unsigned nsteps = 1u << Lw;
-    for (unsigned t = 0; t < nsteps; ++t) {
-        if (t > 0) {
-            // ---- Gray step: flip walk bit k = ctz(t); warp-uniform rows, exact integer updates ----
-            const int k = __ffs(t) - 1;
-            const unsigned gnew = t ^ (t >> 1);
-            const int sb = (gnew >> k) & 1;
-            int phi = PhiW[0];
+    static __device__ __forceinline__ void step(Regs& R, const Shared& sh, int k, int sb)
+    {
+        const int4* dv = reinterpret_cast<const int4*>(sh.DV + (k * 2 + sb) * NLO);
+        const int4* du = reinterpret_cast<const int4*>(sh.DU + (k * 2 + sb) * NMID);
 #pragma unroll
-            for (int kk = 1; kk < LW_MAX; ++kk) phi = (k == kk) ? PhiW[kk] : phi;
-            Eh += sDW[t] + (sb ? -2 * phi : 2 * phi);
-            const int4* dv = reinterpret_cast<const int4*>(sDV + (k * 2 + sb) * NLO);
-            const int4* du = reinterpret_cast<const int4*>(sDU + (k * 2 + sb) * NMID);
-#pragma unroll
-            for (int x = 0; x < NLO / 4; ++x) {
-                const int4 d = dv[x];
-                V[4 * x + 0] += d.x; V[4 * x + 1] += d.y; V[4 * x + 2] += d.z; V[4 * x + 3] += d.w;
-            }
-#pragma unroll
-            for (int x = 0; x < NMID / 4; ++x) {
-                const int4 d = du[x];
-                U[4 * x + 0] += d.x; U[4 * x + 1] += d.y; U[4 * x + 2] += d.z; U[4 * x + 3] += d.w;
-            }
+        for (int x = 0; x < NLO / 4; ++x) {
+            const int4 d = dv[x];
+            R.V[4 * x + 0] += d.x; R.V[4 * x + 1] += d.y; R.V[4 * x + 2] += d.z; R.V[4 * x + 3] += d.w;
         }
-        // ---- a3: 1024 configurations, one add-min each ----
+#pragma unroll
+        for (int x = 0; x < NMID / 4; ++x) {
+            const int4 d = du[x];
+            R.U[4 * x + 0] += d.x; R.U[4 * x + 1] += d.y; R.U[4 * x + 2] += d.z; R.U[4 * x + 3] += d.w;
+        }
+    }
+
+    // a3: 1024 configurations, one add-min each; a4: threshold filter on the exact block minimum; then the Gray step
+    static __device__ __forceinline__ bool hit_step(Regs& R, const Shared& sh, const Tables* __restrict__,
+                                                    int tauE, int Eh, int k, int sb)
+    {
         int g = 0x7fffffff;
 #pragma unroll
         for (int mid = 0; mid < NMID; ++mid) {
-            const int4* crow = reinterpret_cast<const int4*>(sC + mid * NLO);
+            const int4* crow = reinterpret_cast<const int4*>(sh.C + mid * NLO);
             int m = 0x7fffffff;
 #pragma unroll
             for (int x = 0; x < NLO / 4; ++x) {
                 const int4 c = crow[x];
-                m = __viaddmin_s32(V[4 * x + 0], c.x, m);
-                m = __viaddmin_s32(V[4 * x + 1], c.y, m);
-                m = __viaddmin_s32(V[4 * x + 2], c.z, m);
-                m = __viaddmin_s32(V[4 * x + 3], c.w, m);
+                m = __viaddmin_s32(R.V[4 * x + 0], c.x, m);
+                m = __viaddmin_s32(R.V[4 * x + 1], c.y, m);
+                m = __viaddmin_s32(R.V[4 * x + 2], c.z, m);
+                m = __viaddmin_s32(R.V[4 * x + 3], c.w, m);
             }
-            g = __viaddmin_s32(m, U[mid], g);
+            g = __viaddmin_s32(m, R.U[mid], g);
         }
-        // ---- a4: threshold filter; survivors are re-formed by the whole warp, one hit lane at a time ----
-        unsigned hits = __ballot_sync(0xffffffffu, g <= tauE - Eh);
-        while (hits) {
-            const int src = __ffs(hits) - 1;
-            hits &= hits - 1;
-            if (lane == src) {
-#pragma unroll
-                for (int x = 0; x < NLO; ++x) scratch[x] = V[x];
-#pragma unroll
-                for (int x = 0; x < NMID; ++x) scratch[NLO + x] = U[x];
-            }
-            __syncwarp();
-            const int eh = __shfl_sync(0xffffffffu, Eh, src);
-            const unsigned long long qs = q0_warp + ((unsigned long long)src << nlow)
-                                        + ((unsigned long long)(t ^ (t >> 1)) << LOWBITS) + (unsigned)lane;
-            const int v = scratch[lane] + eh;
-            for (int mid = 0; mid < NMID; ++mid) {
-                const int e = v + sC[mid * NLO + lane] + scratch[NLO + mid];
-                const unsigned long long q = qs + ((unsigned)mid << LL);
-                if (e < tauE || (e == tauE && q < tauQ)) push_candidate(ctrl, pool, e, q);
-            }
-            __syncwarp();
-        }
+        step(R, sh, k, sb);
+        return g <= tauE - Eh;
     }
+};
+
+void launch_walk32(const Tables* tab, Ctrl* ctrl, Entry* pool, unsigned* hist, const Plan& plan, cudaStream_t st)
+{
+    // one warp per unit of the plan (the queue hands the units out in ascending q whatever the block order)
+    const unsigned long long blocks = (plan.total_units + WALK_WARPS - 1) / WALK_WARPS;
+    walk_kernel<Inner32><<<(unsigned)blocks, WALK_THREADS, 0, st>>>(tab, ctrl, pool, hist, plan);
 }
 
-// Direct evaluation of eq. (1) on the grid for `count` consecutive states starting at `base`; every state goes to the
-// pool behind the `kept` entries already there. Used for the whole space when N <= N_DIRECT_MAX (2^N <= 16384 states)
-// and for the first 2^15 states of any larger run (a2': with tau = +inf everything passes anyway, and one thread per
-// state is the fastest way to form them).
-__global__ void direct_kernel(const Tables* __restrict__ tab, Ctrl* __restrict__ ctrl, Entry* __restrict__ pool, int N,
-                              unsigned long long base, unsigned count, unsigned kept)
+// Direct evaluation of eq. (1) on the grid for every state of a tiny instance (N <= N_DIRECT_MAX, 2^N <= 16384
+// states): everything goes to the pool (and, in the single-pass path, to the histogram; the last block to finish
+// derives the threshold from it).
+__global__ void direct_kernel(const Tables* __restrict__ tab, Ctrl* __restrict__ ctrl, Entry* __restrict__ pool,
+                              unsigned* __restrict__ hist, int N, int S, unsigned count, int use_hist)
 {
+    if (ctrl->status != 0) return;
+    const long long Wq = ctrl->Wq;
+    const int hs = ctrl->hist_shift;
     for (unsigned t = blockIdx.x * blockDim.x + threadIdx.x; t < count; t += gridDim.x * blockDim.x) {
-        const unsigned long long q = base + t;
+        const unsigned long long q = t;
         int e = 0;
         for (int i = 0; i < N; ++i) {
             const unsigned bi = (unsigned)(q >> i) & 1u;
@@ -195,24 +130,33 @@ __global__ void direct_kernel(const Tables* __restrict__ tab, Ctrl* __restrict__
         Entry en;
         en.key = key_from_i32(e);
         en.q = q;
-        pool[kept + t] = en;
+        pool[t] = en;
+        if (use_hist) {
+            const int b = hist_bin(e, Wq, hs);
+            atomicAdd(hist + HIST_COARSE + b, 1u);
+            atomicAdd(hist + (b >> 8), 1u);
+        }
     }
-    if (blockIdx.x == 0 && threadIdx.x == 0) ctrl->count = kept + count;
+    if (blockIdx.x == 0 && threadIdx.x == 0) ctrl->count = count;
+    if (!use_hist) return;
+    // the last block to finish turns the histogram into the threshold
+    __shared__ int s_last;
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) s_last = atomicAdd(&ctrl->blocks_done, 1u) == gridDim.x - 1;
+    __syncthreads();
+    if (!s_last || threadIdx.x >= 32) return;
+    __threadfence();
+    int tauE;
+    if (hist_threshold(ctrl, hist, (unsigned)S, threadIdx.x, tauE) && threadIdx.x == 0)
+        atomicMin(&ctrl->tau, tau_pack(tauE, QC_NONE));
 }
 
-void launch_enumerate(const Tables* tab, Ctrl* ctrl, Entry* pool, int N, int Lw,
-                      unsigned long long base, unsigned nthreads, cudaStream_t st)
-{
-    const unsigned threads = nthreads < (unsigned)ENUM_THREADS ? nthreads : (unsigned)ENUM_THREADS;
-    const unsigned blocks = (nthreads + threads - 1) / threads;
-    enumerate_kernel<<<blocks, threads, 0, st>>>(tab, ctrl, pool, N, Lw, base, nthreads);
-}
-
-void launch_direct(const Tables* tab, Ctrl* ctrl, Entry* pool, int N, unsigned long long base, unsigned count,
-                   unsigned kept, cudaStream_t st)
+void launch_direct(const Tables* tab, Ctrl* ctrl, Entry* pool, unsigned* hist, int N, int S, unsigned count,
+                   int use_hist, cudaStream_t st)
 {
     const unsigned threads = 128, blocks = (count + threads - 1) / threads;
-    direct_kernel<<<blocks, threads, 0, st>>>(tab, ctrl, pool, N, base, count, kept);
+    direct_kernel<<<blocks, threads, 0, st>>>(tab, ctrl, pool, hist, N, S, count, use_hist);
 }
 
 }  // namespace ising

@@ -97,7 +97,12 @@ __global__ void __launch_bounds__(256) stage_kernel(const double* __restrict__ J
     if (s_status != ISING_OK) { if (tid == 0) ctrl->status = s_status; return; }
     const int p = s_p;
 
-    // ---- quantise; accumulate the rounding error of each weight that enters eq. (1) once ----
+    // ---- quantise; accumulate the rounding error of each weight that enters eq. (1) once, and the exact integer
+    //      sum Wq of the |grid weights| (every grid energy lies in [-Wq, +Wq]) ----
+    __shared__ unsigned long long s_wq;
+    if (tid == 0) s_wq = 0ull;
+    __syncthreads();
+    unsigned long long wq = 0ull;
     double err = 0.0;
     for (int idx = tid; idx < 64 * 64; idx += blockDim.x) {
         int i = idx >> 6, j = idx & 63;
@@ -106,21 +111,23 @@ __global__ void __launch_bounds__(256) stage_kernel(const double* __restrict__ J
             double v = J[i * N + j];
             double r = rint(ldexp(v, p));
             q = (int)r;
-            if (i < j) err += fabs(ldexp(r, -p) - v);
+            if (i < j) { err += fabs(ldexp(r, -p) - v); wq += (unsigned long long)(q < 0 ? -(long long)q : (long long)q); }
         }
         tab->Jq[idx] = q;
     }
     for (int i = tid; i < 64; i += blockDim.x) {
         int q = 0;
         if (i < N) {
-            double v = h[i];
+            double v = FIELD_TERM_SIGN * h[i];                 // the one place the field sign convention enters the grid
             double r = rint(ldexp(v, p));
             q = (int)r;
             err += fabs(ldexp(r, -p) - v);
+            wq += (unsigned long long)(q < 0 ? -(long long)q : (long long)q);
         }
         tab->hq[i] = q;
     }
     s_red[tid] = err;
+    if (wq) atomicAdd(&s_wq, wq);
     __syncthreads();
     for (int s = 128; s > 0; s >>= 1) {
         if (tid < s) s_red[tid] += s_red[tid + s];
@@ -141,12 +148,26 @@ __global__ void __launch_bounds__(256) stage_kernel(const double* __restrict__ J
         ctrl->band = band;
         ctrl->epsilon = eps;
         ctrl->W = W;
+        // histogram of candidate energies (walk.cuh): HIST_FINE bins of 2^hist_shift grid units over [-Wq, +Wq]
+        const long long Wq = (long long)s_wq;
+        int hs = 0;
+        while (((2 * Wq) >> hs) >= (long long)HIST_FINE) ++hs;
+        ctrl->Wq = Wq;
+        ctrl->hist_shift = hs;
         ctrl->count = 0;
         ctrl->kept = 0;
-        ctrl->tauE = TAU_INF;
-        ctrl->tauQ = Q_MAX;
+        ctrl->tau = tau_pack(TAU_INF, QC_NONE);
         ctrl->band_overflow = 0;
-        ctrl->candidates = 0;
+        ctrl->pool_overflow = 0;
+        ctrl->next_unit = 0ull;
+        ctrl->done_configs = 0ull;
+        ctrl->count2 = 0;
+        ctrl->final_state = 0;
+        ctrl->eS = 0;
+        ctrl->n_sure = 0;
+        ctrl->blocks_done = 0;
+        ctrl->hits = 0ull;
+        ctrl->false_hits = 0ull;
     }
 }
 
@@ -286,7 +307,7 @@ __global__ void qubo_to_ising_kernel(const double* __restrict__ a, const double*
     for (int i = threadIdx.x; i < N; i += blockDim.x) {
         double acc = 0.0;
         for (int j = 0; j < N; ++j) if (j != i) acc += a[i * N + j];
-        h[i] = 0.5 * b[i] + 0.25 * acc;
+        h[i] = FIELD_TERM_SIGN * (0.5 * b[i] + 0.25 * acc);
     }
 }
 void launch_qubo_to_ising(const double* a, const double* b, int N, double* J, double* h, cudaStream_t st)
