@@ -4,14 +4,18 @@ A "step" is ONE full pass of the hot path over one instance: all 2^48 spin confi
 selected, the survivors re-evaluated in fp64 and the S lowest written.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config k] [--range-log2 r]
+                    [--weak] [--n-spins 50|52]
 
-  value        configurations evaluated per second, whole job, inputs resident in HBM, CUDA-event timed
-  e2e          same through ising_lowest_host: pinned HOST buffers in and out, copies inside the timed region
-  roofline     the enumeration kernel against the integer add-min ceiling
-  cpu_baseline the CPU oracle, as it stands, on a bounded prefix of the same instance (rank 0, N=1 only)
+  value          configurations evaluated per second, whole job, inputs resident in HBM, CUDA-event timed
+  e2e            same through the host-buffer API: pinned HOST buffers in and out, copies inside the timed region
+  roofline       the enumeration kernel (packed 16-bit screen) against the MEASURED rate of its instruction mix
+  roofline_int32 the int32 kernel (arithmetic no narrower than the paper's) on the same full space, same invocation
+  cpu_baseline   the CPU oracle, as it stands, on a bounded prefix of the same instance (rank 0, N=1 only)
 
-N > 1 (torchrun): the path shards over independent problems -- one seeded instance per rank, no data-path
-collective -- so scaling is "weak" and value = N * 2^48 / (max over ranks of the device time).
+N > 1 (torchrun): the path shards by ranges of q: ONE instance, one aligned state range per rank,
+one all-gather of the per-rank lists, merge on every rank -- "strong" scaling, value = 2^N / (max over ranks of the
+device time). --n-spins 50|52 swaps in a complete Gaussian instance of that size so that 8 ranks have seconds of
+work each. --weak keeps the other reading (independent instances per rank, no data-path collective).
 --impl reference times the CPU oracle (there is no other reference implementation in this tier).
 """
 from __future__ import annotations
@@ -53,17 +57,25 @@ def parse_args():
     ap.add_argument("--range-log2", type=int, default=0,
                     help="development only: enumerate just the first 2^r states per step (0 = the whole space)")
     ap.add_argument("--sharded", action="store_true",
-                    help="N > 1: ONE instance, its state space cut into one aligned range per rank, lists exchanged with "
-                         "an all-gather and merged (paper_1904_03621_b200/sharded.py): strong scaling. Default: every "
-                         "rank enumerates its own instance (weak scaling, no data-path collective)")
+                    help="go through paper_1904_03621_b200/sharded.py even with one rank (default for N > 1): ONE "
+                         "instance, one aligned state range per rank, one all-gather, merge on every rank")
+    ap.add_argument("--weak", action="store_true",
+                    help="N > 1: every rank enumerates its own instance of the ensemble (weak scaling, no collective)")
+    ap.add_argument("--n-spins", type=int, default=0,
+                    help="replace the config's instance by a complete Gaussian instance of this many spins (S as in the "
+                         "config); for multi-GPU runs, e.g. 50 or 52")
+    ap.add_argument("--no-int32", action="store_true", help="skip the int32-kernel pass (one more full enumeration)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
 
 
-def instance_for_rank(k: int, rank: int):
+def instance_for_rank(k: int, rank: int, n_spins: int = 0):
     from paper_1904_03621_b200 import instances as I
     c = I.baseline_config(k)
+    if n_spins:
+        J, h = I.complete_gaussian(n_spins, I.SEED_BASE + 100 * n_spins + 1000 * rank)
+        return I.Instance(f"complete_gauss_N{n_spins}_rank{rank}", n_spins, c.S, J, h, False)
     if rank == 0:
         return c
     # other ranks: an independent instance of the same ensemble (same generator, rank-specific seed)
@@ -157,7 +169,7 @@ def run_reference(args, rank: int, world: int):
     if rank != 0:
         return
     from oracle import oracle
-    inst = instance_for_rank(args.config, 0)
+    inst = instance_for_rank(args.config, 0, args.n_spins)
     cores = oracle.max_threads()
     # size one step for roughly 3 s of oracle time
     rate, _, kk, _ = oracle_sample_rate(inst, 3.0, inst.S)
@@ -210,8 +222,10 @@ def main():
         dist.barrier()
     B.load()
 
-    sharded_mode = args.sharded and world > 1
-    inst = instance_for_rank(args.config, 0 if sharded_mode else rank)
+    # N > 1: range-sharded on ONE instance unless --weak; N = 1: the plain call (or, with --sharded,
+    # the same call through sharded.py, which must give the same number)
+    sharded_mode = (world > 1 and not args.weak) or args.sharded
+    inst = instance_for_rank(args.config, 0 if sharded_mode else rank, args.n_spins)
     N, S = inst.N, inst.S
     q_end = 1 << N
     if args.range_log2:
@@ -222,11 +236,14 @@ def main():
     out = (torch.empty(S, dtype=torch.int64, device="cuda"), torch.empty(S, dtype=torch.float64, device="cuda"))
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")          # > 126 MB L2
     stream = torch.cuda.current_stream()
+    if sharded_mode and args.range_log2:
+        raise SystemExit("--range-log2 is a single-range development knob; it cannot be combined with the sharded mode")
 
     def step():
         if sharded_mode:
             from paper_1904_03621_b200 import sharded
-            sharded.ising_lowest_sharded(J, h, S)          # every rank ends with the global list
+            res = sharded.ising_lowest_sharded(J, h, S)    # every rank ends with the global list
+            out[0].copy_(res[0]); out[1].copy_(res[1])
         else:
             B.ising_lowest_range(J, h, S, 0, q_end, stream=stream, out=out)
         return B.last_stats()
@@ -240,6 +257,7 @@ def main():
     fma_peak = B.fma_peak(50.0)
     addmin_peak = B.addmin_peak(50.0)
     addmin16x2_peak = B.addmin16x2_peak(50.0)
+    addmin_mix_peak = B.addmin_mix_peak(50.0)
 
     for _ in range(args.warmup):
         flush.zero_()
@@ -255,6 +273,7 @@ def main():
     enum_launches = 0
     launches = 0
     enum_configs = 0
+    hit_blocks = false_hit_blocks = 0
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     for _ in range(args.steps):
         flush.zero_()                       # L2 flush between timed iterations (outside the event bracket)
@@ -267,13 +286,17 @@ def main():
         enum_configs += st.configs
         enum_launches += st.enum_launches
         launches += st.kernel_launches
+        hit_blocks += st.hit_blocks
+        false_hit_blocks += st.false_hit_blocks
     barrier()
     t_wall1 = time.perf_counter()
     clocks = sampler.summary(t_wall0, t_wall1)
+    result_states = B.states_to_numpy(out[0]).tolist()
 
-    # ---- end to end: pinned host buffers in, host buffers out, through ising_lowest_host ----
+    # ---- end to end: pinned host buffers in, host buffers out (ising_lowest_host; sharded: the same call through
+    # sharded.py with the host arrays, every rank copying its result back to the host) ----
     e2e = None
-    if not args.no_e2e and not sharded_mode:
+    if not args.no_e2e:
         Jh = torch.from_numpy(inst.J).pin_memory()
         hh = torch.from_numpy(inst.h).pin_memory()
         qh = torch.empty(S, dtype=torch.int64).pin_memory()
@@ -282,11 +305,38 @@ def main():
         barrier()
         t0 = time.perf_counter()
         for _ in range(args.steps):
-            B.ising_lowest_host(Jh.numpy(), hh.numpy(), S, 0, q_end, stream=stream, out=out_h)
-        torch.cuda.synchronize()
+            if sharded_mode:
+                from paper_1904_03621_b200 import sharded
+                rq, re_ = sharded.ising_lowest_sharded(Jh.numpy(), hh.numpy(), S)   # H2D of J, h inside the solver call
+                qh.copy_(rq, non_blocking=True); eh.copy_(re_, non_blocking=True)
+                torch.cuda.synchronize()
+            else:
+                B.ising_lowest_host(Jh.numpy(), hh.numpy(), S, 0, q_end, stream=stream, out=out_h)
+        barrier()
         e2e_s = time.perf_counter() - t0
-        assert qh.numpy().view(np.uint64).tolist() == B.states_to_numpy(out[0]).tolist()
+        assert qh.numpy().view(np.uint64).tolist() == result_states
         e2e = {"seconds": e2e_s, "h2d": (N * N + N) * 8, "d2h": S * 16}
+
+    # ---- the int32 kernel (32-bit exact add-min per configuration: no narrower than the paper's arithmetic) on the
+    # same workload, timed with its own CUDA events; fewer steps (it is 2.2x slower), rank-local like `roofline` ----
+    int32 = None
+    if not args.no_int32 and not sharded_mode:
+        os.environ["ISING_KERNEL"] = "32"
+        try:
+            n32 = max(1, min(args.steps, 2))
+            ms32 = e32 = 0.0
+            c32 = 0
+            for _ in range(n32):
+                ev0.record(stream)
+                q32, _ = B.ising_lowest_range(J, h, S, 0, q_end, stream=stream)
+                ev1.record(stream); ev1.synchronize()
+                st32 = B.last_stats()
+                assert st32.kernel_variant == 32
+                ms32 += ev0.elapsed_time(ev1); e32 += st32.enum_ms; c32 += st32.configs
+            assert B.states_to_numpy(q32).tolist() == result_states       # same list as the packed kernel
+            int32 = {"ms_per_step": ms32 / n32, "enum_ms": e32, "configs": c32, "steps": n32}
+        finally:
+            os.environ.pop("ISING_KERNEL", None)
     sampler.stop()
 
     # max over ranks of the device time
@@ -306,63 +356,79 @@ def main():
             pass
         sms = torch.cuda.get_device_properties(local_rank).multi_processor_count
         per_inst = 2 if st.kernel_variant == 16 else 1                 # add-mins (configurations) per lane instruction
-        fused_peak = sms * ALU_LANES_PER_CLK_PER_SM * sm_max_hz * per_inst         # add-min ops / s, fused form only
+        fused_nominal = sms * ALU_LANES_PER_CLK_PER_SM * sm_max_hz * per_inst     # add-min ops / s, fused form only
         fused_live = addmin16x2_peak * 2 if st.kernel_variant == 16 else addmin_peak
-        if st.kernel_variant == 16:
-            alu_peak = sms * MIX_BOUND_CONFIGS_PER_CLK_PER_SM * sm_max_hz
-            live_peak = fused_live * MIX_BOUND_CONFIGS_PER_CLK_PER_SM / (ALU_LANES_PER_CLK_PER_SM * per_inst)
-        else:
-            alu_peak, live_peak = fused_peak, fused_live
-        kname = "ising::enumerate16_kernel" if st.kernel_variant == 16 else "ising::enumerate_kernel"
+        derived_mix = sms * MIX_BOUND_CONFIGS_PER_CLK_PER_SM * sm_max_hz
+        # the peak the fraction is quoted against is MEASURED in this run: for the packed kernel the best of the two
+        # register-only microbenchmarks of its own instruction forms (fused VIADDMNMX.U16x2 alone; fused + split mix)
+        peak_live = max(fused_live, addmin_mix_peak) if st.kernel_variant == 16 else fused_live
+        kname = "ising::walk_kernel<Inner16>" if st.kernel_variant == 16 else "ising::walk_kernel<Inner32>"
         fma_nominal = sms * FMA_LANES_PER_CLK_PER_SM * sm_max_hz       # FMA / s
         achieved = float(enum_configs) / (enum_ms * 1e-3)   # this rank's kernel: one add-min per configuration
-        traffic = None
+        traffic, traffic_source = None, None
         tpath = os.path.join(ROOT, "profiles", "enumerate_dram_bytes_per_launch.txt")
         if os.path.exists(tpath):
             try:
-                traffic = float(open(tpath).read().split()[0])
+                txt = open(tpath).read().split()
+                traffic = float(txt[0])
+                traffic_source = ("ncu --set full capture of one launch of this kernel (dram__bytes_read.sum + "
+                                  "dram__bytes_write.sum), stored in profiles/enumerate_dram_bytes_per_launch.txt; "
+                                  "not re-measured in this run")
             except Exception:
                 traffic = None
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": dev_ms_max / args.steps, "higher_is_better": True,
-            "scaling": "strong" if sharded_mode else "weak", "vs_baseline": None,
+            "scaling": "strong" if (sharded_mode and world > 1) else "weak", "vs_baseline": None,
             "dtype": "int16x2 screen + int32 exact (fp64 output)" if st.kernel_variant == 16 else "int32 (fp64 output)",
             "data": "synthetic",
             "config": {"workload": f"BASELINE.json configs[{args.config - 1}]: {inst.name}, N={N}, S={S}, "
                                    f"states [0, 2^{q_end.bit_length() - 1}) of 2^{N} per step",
-                       "parallelism": (f"one instance, {world} state ranges + all-gather + merge" if sharded_mode else
+                       "instance_sha256": inst.sha256(),
+                       "parallelism": (f"one instance, {world} state range(s) + one all-gather + merge (sharded.py)"
+                                       if sharded_mode else
                                        f"independent instances x{world}" if world > 1 else "single GPU"),
                        "l2": "256 MiB buffer written between timed steps (inputs are 18 KB; the path has no HBM traffic)",
                        "grid_exponent_p": st.grid_exponent, "epsilon": st.epsilon, "kept": st.keep,
                        "kernel_variant": st.kernel_variant, "screen_shift": st.screen_shift,
-                       "candidates": st.candidates},
+                       "candidates": st.candidates, "passes": st.passes,
+                       "screened_blocks_formed_exactly": hit_blocks, "of_which_false_hits": false_hit_blocks},
             "time_to_S_lowest_s": dev_ms_max * 1e-3 / args.steps,
             "fp32_fma_roofline": {"definition": "configs/s x N / peak FP32 FMA/s (BASELINE.json metric)",
                                   "frac_of_measured": value / world * N / fma_peak,
                                   "frac_of_nominal": value / world * N / fma_nominal,
                                   "fma_per_s_measured": fma_peak, "fma_per_s_nominal": fma_nominal},
-            "roofline": {"bound": "alu", "achieved": achieved, "peak": alu_peak, "unit": "add-min/s",
-                         "frac": achieved / alu_peak, "traffic": traffic,
+            "roofline": {"bound": "alu", "achieved": achieved, "peak": peak_live, "unit": "add-min/s",
+                         "frac": achieved / peak_live, "traffic": traffic, "traffic_source": traffic_source,
                          "kernel": kname, "launches": enum_launches,
                          "avg_launch_ms": enum_ms / max(enum_launches, 1),
-                         "peak_source": ("derived: SMs x 192 add-min/clk (ALU pipe 16 lanes/clk and 1 issue slot/clk per "
-                                         "sub-partition; best mix of VIADDMNMX.U16x2 and IMAD+IMAD+VIMNMX3.U16x2) "
-                                         "x sm_max_mhz of MEASURED_PEAKS.json (DESIGN.md 5.2)"
-                                         if st.kernel_variant == 16 else
-                                         "derived: SMs x 64 ALU lanes/clk x 1 add-min per lane instruction "
-                                         "x sm_max_mhz of MEASURED_PEAKS.json (DESIGN.md 5.2)"),
-                         "peak_measured_live": live_peak, "frac_of_measured_live": achieved / live_peak,
-                         "fused_only_ceiling": fused_peak, "frac_of_fused_only_ceiling": achieved / fused_peak,
-                         "fused_only_ceiling_measured_live": fused_live,
+                         "peak_source": ("MEASURED in this run: max of ising_addmin16x2_peak x 2 (fused VIADDMNMX.U16x2 "
+                                         "only) and ising_addmin_mix_peak (fused + IMAD/IMAD/VIMNMX3.U16x2 mix), "
+                                         "register-only loops on the whole GPU" if st.kernel_variant == 16 else
+                                         "MEASURED in this run: ising_addmin_peak (VIADDMNMX.S32, register-only loop)"),
+                         "fused_only_measured": fused_live, "mix_measured": addmin_mix_peak,
+                         "fused_only_nominal": fused_nominal, "frac_of_fused_only_nominal": achieved / fused_nominal,
+                         "mix_bound_derived": derived_mix, "frac_of_mix_bound_derived": achieved / derived_mix,
+                         "mix_bound_note": "derived LP bound (ALU pipe 16 lanes/clk, 1 issue slot/clk per sub-partition); "
+                                           "the measured mix does not reach it: VIMNMX3.U16x2 and IMAD do not overlap "
+                                           "with VIADDMNMX as the LP assumes (DESIGN.md 5.2)",
                          "viaddmnmx_s32_per_s_live": addmin_peak, "viaddmnmx_u16x2_per_s_live": addmin16x2_peak},
             "gpu_launches": launches,
             "clocks": clocks,
         }
+        if int32:
+            a32 = float(int32["configs"]) / (int32["enum_ms"] * 1e-3)
+            line["roofline_int32"] = {"bound": "alu", "kernel": "ising::walk_kernel<Inner32>", "achieved": a32,
+                                      "peak": addmin_peak, "unit": "add-min/s", "frac": a32 / addmin_peak,
+                                      "peak_source": "MEASURED in this run: ising_addmin_peak (VIADDMNMX.S32)",
+                                      "time_to_S_lowest_s": int32["ms_per_step"] * 1e-3,
+                                      "configs_per_s": float(configs_per_step) / (int32["ms_per_step"] * 1e-3),
+                                      "steps": int32["steps"], "same_list_as_packed_kernel": True,
+                                      "dtype": "int32 (fp64 output)"}
         if e2e:
             line["e2e"] = {"value": total_configs / e2e_s_max, "unit": UNIT,
                            "h2d_bytes_per_step": e2e["h2d"], "d2h_bytes_per_step": e2e["d2h"]}
-        if world == 1 and not args.range_log2:
+        if world == 1 and not args.range_log2 and not args.n_spins:
             # north_star: configs/s and time-to-solution for every BASELINE.json config (the other four are
             # parity-test cases, reported here for reference only: median of 5 whole-space calls, CUDA events)
             per = []
@@ -380,11 +446,29 @@ def main():
                 per.append({"config": k, "name": ck.name, "N": ck.N, "S": ck.S, "time_to_S_lowest_ms": ms,
                             "configs_per_s": float(1 << ck.N) / (ms * 1e-3), "exact": bool(stk.exact),
                             "screen_shift": stk.screen_shift, "candidates": stk.candidates,
+                            "kernel_launches": stk.kernel_launches,
                             "fp32_fma_roofline_frac": float(1 << ck.N) / (ms * 1e-3) * ck.N / fma_peak})
             per.append({"config": 5, "name": inst.name, "N": N, "S": S, "time_to_S_lowest_ms": dev_ms_max / args.steps,
                         "configs_per_s": value, "exact": bool(st.exact), "screen_shift": st.screen_shift,
-                        "candidates": st.candidates, "fp32_fma_roofline_frac": value * N / fma_peak})
+                        "candidates": st.candidates, "kernel_launches": st.kernel_launches,
+                        "fp32_fma_roofline_frac": value * N / fma_peak})
             line["per_config"] = per
+            # "time proportional to 2^N": complete Gaussian instances N = 24 .. 44, configs/s of the whole call
+            sweep = []
+            for n in (24, 28, 32, 36, 40, 44):
+                from paper_1904_03621_b200 import instances as I
+                Jn, hn = I.complete_gaussian(n, I.SEED_BASE + 100 * n)
+                Jn = torch.from_numpy(Jn).cuda(); hn = torch.from_numpy(hn).cuda()
+                ts = []
+                for _ in range(3 if n >= 40 else 5):
+                    ev0.record(stream)
+                    B.ising_lowest(Jn, hn, 100, stream=stream)
+                    ev1.record(stream); ev1.synchronize()
+                    ts.append(ev0.elapsed_time(ev1))
+                ms = sorted(ts[1:])[len(ts[1:]) // 2]
+                sweep.append({"N": n, "S": 100, "ms": ms, "configs_per_s": float(1 << n) / (ms * 1e-3)})
+            sweep.append({"N": N, "S": S, "ms": dev_ms_max / args.steps, "configs_per_s": value})
+            line["n_sweep_complete_gaussian"] = sweep
             # the paper's own pipeline (Algorithm 1) written plainly for this GPU, on a 2^28-state slice of the same
             # instance: the on-box "prior design" figure; not a target, not the reference arm
             n_alg1 = 1 << min(28, N)

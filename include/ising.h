@@ -168,6 +168,8 @@ typedef struct ising_stats {
     int32_t  kernel_variant;     /* 1: ising_lowest_alg1. 2: ising_dos. 16: packed 16-bit screen + exact int32 re-forming of hit blocks (default);
                                     32: int32 add-min per configuration (environment ISING_KERNEL=32) */
     int32_t  screen_shift;       /* variant 16: one 16-bit unit = 2^screen_shift grid units (0: screen is exact) */
+    uint64_t hit_blocks;         /* 1024-configuration blocks that passed the screen and were formed exactly (int32) */
+    uint64_t false_hit_blocks;   /* ... of which none held a candidate (the price of the 16-bit screen; 0 for variant 32) */
 } ising_stats;
 
 int ising_get_last_stats(ising_stats *out_host);

@@ -39,7 +39,8 @@ class _Stats(ctypes.Structure):
                 ("grid_exponent", ctypes.c_int32), ("exact", ctypes.c_int32),
                 ("epsilon", ctypes.c_double), ("enum_ms", ctypes.c_double), ("total_ms", ctypes.c_double),
                 ("keep", ctypes.c_int32), ("inner_bits", ctypes.c_int32),
-                ("kernel_variant", ctypes.c_int32), ("screen_shift", ctypes.c_int32)]
+                ("kernel_variant", ctypes.c_int32), ("screen_shift", ctypes.c_int32),
+                ("hit_blocks", ctypes.c_uint64), ("false_hit_blocks", ctypes.c_uint64)]
 
 
 @dataclass
@@ -59,6 +60,8 @@ class Stats:
     inner_bits: int
     kernel_variant: int
     screen_shift: int
+    hit_blocks: int = 0
+    false_hit_blocks: int = 0
 
 
 _lib = None
@@ -147,7 +150,8 @@ def last_stats() -> Stats:
     s = _Stats()
     _check(load().ising_get_last_stats(ctypes.byref(s)), "ising_get_last_stats")
     return Stats(s.configs, s.candidates, s.kernel_launches, s.enum_launches, s.passes, s.split_retries,
-                 s.grid_exponent, bool(s.exact), s.epsilon, s.enum_ms, s.total_ms, s.keep, s.inner_bits, s.kernel_variant, s.screen_shift)
+                 s.grid_exponent, bool(s.exact), s.epsilon, s.enum_ms, s.total_ms, s.keep, s.inner_bits, s.kernel_variant, s.screen_shift,
+                 s.hit_blocks, s.false_hit_blocks)
 
 
 def ising_lowest_range(J, h, S: int, q_begin: int, q_end: int, stream=None, out=None):

@@ -163,6 +163,7 @@ struct Run {
     unsigned long long q_begin, q_end;
     cudaStream_t st;
     double enum_ms;
+    bool done;                      // the single pass wrote the outputs and recorded the end event
 };
 
 void plan_header(const Run& r, Plan& plan, int use_hist, int loE)
@@ -183,7 +184,10 @@ void plan_header(const Run& r, Plan& plan, int use_hist, int loE)
 // Walk-bit count of a segment of sz configurations at cur: enough units to balance the persistent warps, aligned.
 int choose_lw(unsigned long long cur, unsigned long long sz, int lw_max)
 {
-    int Lw = floor_log2(sz) - MIN_CHUNK_BITS - 12;
+    // about 2^11 units per segment: a unit costs about two Gray steps to set up (queue, base state, tables), so short
+    // units are expensive (measured on cfg2: 2^13 units per segment 0.59 ms, 2^12 0.55 ms, 2^11 0.49 ms per call);
+    // the tail of the last segment is tapered instead (run_single_pass)
+    int Lw = floor_log2(sz) - MIN_CHUNK_BITS - 11;
     Lw = Lw < 0 ? 0 : (Lw > lw_max ? lw_max : Lw);
     while (Lw > 0 && (cur & ((1ull << (MIN_CHUNK_BITS + Lw)) - 1ull))) --Lw;
     return Lw;
@@ -217,7 +221,6 @@ int run_single_pass(Run& r, unsigned long long* states_out, double* energies_out
     *redo = false;
     Plan plan;
     plan_header(r, plan, 1, INT32_MIN);
-    CUDA_TRY(cudaMemsetAsync(ws.hist, 0, sizeof(unsigned) * (size_t)HIST_WORDS, r.st));
     const unsigned long long range = r.q_end - r.q_begin;
     const bool direct = r.N <= N_DIRECT_MAX;
     CUDA_TRY(cudaEventRecord(ws.ev[2], r.st));
@@ -281,6 +284,7 @@ int run_single_pass(Run& r, unsigned long long* states_out, double* energies_out
     r.stats->kernel_launches += launch_final_small(r.mode ? r.Jorig : r.J, r.mode ? r.horig : r.h, r.N, r.mode, ws.pool2,
                                                    ws.ctrl, r.S, r.keep_cap, states_out, energies_out, r.st);
     LAUNCH_CHECK("final_small_kernel");
+    CUDA_TRY(cudaEventRecord(ws.ev[1], r.st));          // end of the call if the one-block selection sufficed
     int rc = read_ctrl(r);
     if (rc != ISING_OK) return rc;
     float ms = 0.f;
@@ -291,7 +295,7 @@ int run_single_pass(Run& r, unsigned long long* states_out, double* energies_out
     r.stats->configs += range;
     if (c.pool_overflow) { *redo = true; return ISING_OK; }
     r.stats->candidates += c.count;
-    if (c.final_state == 1) { r.stats->keep = (int)c.kept; return ISING_OK; }
+    if (c.final_state == 1) { r.stats->keep = (int)c.kept; r.done = true; return ISING_OK; }
     if (c.final_state != 2 || c.count2 < (unsigned)r.S) {
         t_last_error = "internal: fewer candidates than requested states";
         return ISING_ERR_INTERNAL;
@@ -346,7 +350,7 @@ int run_pieces(Run& r, bool band_mode, int loE, unsigned want)
             cur += 1ull << MIN_CHUNK_BITS;
         } else {
             const unsigned long long remaining = r.q_end - cur;
-            unsigned long long target = band_mode ? (1ull << r.chunk_log2) : (unsigned long long)r.growth * 3ull * processed;
+            unsigned long long target = band_mode ? (1ull << r.chunk_log2) : (unsigned long long)r.growth * processed;
             if (target > (1ull << r.chunk_log2)) target = 1ull << r.chunk_log2;
             if (!tau_finite && target > (1ull << 16)) target = 1ull << 16;     // everything passes: keep it small
             if (target < (1ull << MIN_CHUNK_BITS)) target = 1ull << MIN_CHUNK_BITS;
@@ -434,20 +438,20 @@ int run_lowest(const double* J, const double* h, const double* Jorig, const doub
     r.mode = mode; r.N = N; r.S = S;
     r.lw_max = env_int("ISING_LW", LW_MAX, 0, LW_MAX);
     r.chunk_log2 = env_int("ISING_CHUNK_LOG2", 42, MIN_CHUNK_BITS, 44);
-    r.growth = env_int("ISING_GROWTH", 1, 1, 1 << 20);      // a segment is at most growth x what lies before it
+    r.growth = env_int("ISING_GROWTH", 3, 1, 1 << 20);      // a segment is at most growth x what lies before it
     r.variant = env_int("ISING_KERNEL", 16, 16, 32) == 32 ? 32 : 16;   // 16: packed screen, 32: int32 kernel
     // test knob for the band pass: a selection keeps at most 2^k entries (never fewer than S)
     r.keep_cap = 1u << env_int("ISING_KEEP_CAP_LOG2", 20, 5, 20);
     while (r.keep_cap < (unsigned)S) r.keep_cap <<= 1;
     const int path = env_int("ISING_PATH", 0, 0, 1);        // 1: skip the single pass (tests of the host-sequenced path)
-    r.q_begin = q_begin; r.q_end = q_end; r.st = st; r.enum_ms = 0.0;
+    r.q_begin = q_begin; r.q_end = q_end; r.st = st; r.enum_ms = 0.0; r.done = false;
     const int rb = floor_log2(q_end - q_begin - 1) + 1;     // bits of the range
     r.qshift = rb > 31 ? rb - 31 : 0;                       // (range >> qshift) < 2^32 - 1
 
     CUDA_TRY(cudaEventRecord(ws.ev[0], st));
-    launch_stage(J, h, N, ws.tab, ws.ctrl, st, extra_eps_rel);
-    LAUNCH_CHECK("stage kernels");
-    stats.kernel_launches += 2;
+    launch_stage(J, h, N, ws.tab, ws.ctrl, ws.hist, st, extra_eps_rel);
+    LAUNCH_CHECK("stage_kernel");
+    stats.kernel_launches += 1;
     stats.inner_bits = LOWBITS;
     stats.kernel_variant = r.variant;
     stats.passes = 1;
@@ -523,13 +527,17 @@ int run_lowest(const double* J, const double* h, const double* Jorig, const doub
                                                   states_out, energies_out, st);
         LAUNCH_CHECK("final kernels");
     }
-    CUDA_TRY(cudaEventRecord(ws.ev[1], st));
-    CUDA_TRY(cudaStreamSynchronize(st));
+    if (!r.done) {
+        CUDA_TRY(cudaEventRecord(ws.ev[1], st));
+        CUDA_TRY(cudaStreamSynchronize(st));
+    }
     CUDA_TRY(cudaGetLastError());
     float total_ms = 0.f;
     CUDA_TRY(cudaEventElapsedTime(&total_ms, ws.ev[0], ws.ev[1]));
     stats.enum_ms = r.enum_ms;
     stats.total_ms = total_ms;
+    stats.hit_blocks = ws.h_ctrl->hits;
+    stats.false_hit_blocks = ws.h_ctrl->false_hits;
     t_stats = stats;
     t_have_stats = true;
     return ISING_OK;
@@ -616,8 +624,8 @@ int ising_dos(const double* J_dev, const double* h_dev, int N, int nbins, uint64
     ising_stats stats;
     memset(&stats, 0, sizeof(stats));
     CUDA_TRY(cudaEventRecord(ws.ev[0], st));
-    launch_stage(J_dev, h_dev, N, ws.tab, ws.ctrl, st, 0.0);
-    stats.kernel_launches += 2;
+    launch_stage(J_dev, h_dev, N, ws.tab, ws.ctrl, nullptr, st, 0.0);
+    stats.kernel_launches += 1;
     CUDA_TRY(cudaMemcpyAsync(ws.h_ctrl, ws.ctrl, sizeof(Ctrl), cudaMemcpyDeviceToHost, st));
     CUDA_TRY(cudaStreamSynchronize(st));
     if (ws.h_ctrl->status != ISING_OK) {
@@ -684,8 +692,8 @@ int ising_lowest_alg1(const double* J_dev, const double* h_dev, int N, int S, ui
     ising_stats stats;
     memset(&stats, 0, sizeof(stats));
     CUDA_TRY(cudaEventRecord(ws.ev[0], st));
-    launch_stage(J_dev, h_dev, N, ws.tab, ws.ctrl, st, 0.0);          // validation only (same error codes)
-    stats.kernel_launches += 2;
+    launch_stage(J_dev, h_dev, N, ws.tab, ws.ctrl, nullptr, st, 0.0);          // validation only (same error codes)
+    stats.kernel_launches += 1;
     CUDA_TRY(cudaMemcpyAsync(ws.h_ctrl, ws.ctrl, sizeof(Ctrl), cudaMemcpyDeviceToHost, st));
     CUDA_TRY(cudaStreamSynchronize(st));
     if (ws.h_ctrl->status != ISING_OK && ws.h_ctrl->status != ISING_ERR_RANGE_W) {

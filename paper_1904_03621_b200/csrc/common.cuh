@@ -167,7 +167,7 @@ struct Plan {
 };
 
 // stage.cu
-void launch_stage(const double* J, const double* h, int N, Tables* tab, Ctrl* ctrl, cudaStream_t st,
+void launch_stage(const double* J, const double* h, int N, Tables* tab, Ctrl* ctrl, unsigned* hist, cudaStream_t st,
                   double extra_eps_rel);
 void launch_qubo_to_ising(const double* a, const double* b, int N, double* J, double* h, cudaStream_t st);
 // enumerate.cu / enumerate16.cu: the persistent enumeration kernel, int32 and packed 16-bit variants

@@ -25,10 +25,11 @@
 //   * a Gray step updates the packed tables with 32-bit adds of the packed delta (d_lo + 65536 d_hi);
 //   * the first sum of every row and the two sums of every row fold are plain adds; the fold's minimum of three is
 //     ONE VIMNMX3.U16x2;
-//   * in the last P1_CHUNKS of the 8 chunks of a row the sums are plain adds and one VIMNMX3.U16x2 takes the minimum
+//   * in three of the 8 chunks of a row (E16_P1MASK) the sums are plain adds and one VIMNMX3.U16x2 takes the minimum
 //     of two of them: 4 configurations per ALU instruction instead of 2, for one more issue slot per two sums.
-//     Measured on B200 (2^45-state slice of cfg5): P1_CHUNKS = 0: 3.25e13/s, 1: 3.39e13, 2: 3.42e13, 3: 3.41e13,
-//     4: 3.41e13, 5: 3.29e13 -- beyond 2 the issue slots, not the ALU pipe, become the limit.
+//     The measured rate of this instruction mix in isolation (ising_addmin_mix_peak) is NOT above the fused form's
+//     (VIMNMX3.U16x2 issues at the same 2 cycles per warp as VIADDMNMX.U16x2 and does not overlap with it); what
+//     the split chunks buy is scheduling slack, a few per cent (table in hit_step below).
 //
 // Walk: as in enumerate.cu (reflected Gray code over the Lw walk bits). The walked 16-bit tables are
 // V16 = floor(V(q0)/2^s) + sum over SET walk bits k of floor(DV_on[k]/2^s): turning a bit off subtracts exactly what
@@ -112,11 +113,16 @@ struct Inner16 {
 
     // a3: 1024 configurations, one packed add-min per two of them; a4: the screen on the lower bound,
     //   bound * 2^s + Eh <= tauE  <=>  bound <= (tauE - Eh) >> s
+    // Which of the chunks 1..7 of a row use the split form (bit x of E16_P1MASK), and the statement order of the two
+    // register sets inside a fused chunk (E16_ORDER), decide how ptxas schedules the loop. Measured on B200, 2^43-state
+    // slice of cfg5, configurations/s (all variants have 0 register-bank conflicts):
+    //   mask 0xC0: 3.34e13   0x06: 3.39e13   0x82: 3.36e13   0x60: 3.25e13   0x80: 3.27e13   0xE0: 3.42e13   0x46: 3.40e13
+    //   0x1E: 3.37e13   0xF0: 3.29e13   0xAA: 3.30e13   0xE0 + order 1: 3.45e13 (default)   0xE0 + order 2: 3.41e13
 #ifndef E16_ORDER
-#define E16_ORDER 0
+#define E16_ORDER 1
 #endif
 #ifndef E16_P1MASK
-#define E16_P1MASK 0xC0          // chunks 6 and 7 of every row in the split form (P1_CHUNKS = 2)
+#define E16_P1MASK 0xE0          // chunks 5, 6 and 7 of every row in the split form
 #endif
     // ... and the Gray step that follows (walk bit k turns on/off): the V tables are updated chunk by chunk right after
     // their last use in the last row, so that the 80 table adds and their loads overlap the add-mins instead of forming

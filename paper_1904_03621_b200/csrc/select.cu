@@ -409,12 +409,14 @@ __global__ void __launch_bounds__(SORT_THREADS) final_small_kernel(const double*
     }
     __syncthreads();
     const unsigned keep = s_keep;
-    for (int i = threadIdx.x; i < tile; i += blockDim.x) {
+    int tile2 = 32;                                    // the kept entries are the first `keep` of the sorted tile
+    while ((unsigned)tile2 < keep) tile2 <<= 1;
+    for (int i = threadIdx.x; i < tile2; i += blockDim.x) {
         if ((unsigned)i < keep) s[i].key = key_from_f64(energy_f64(J, h, N, s[i].q, mode));
         else { s[i].key = ~0ull; s[i].q = ~0ull; }
     }
     __syncthreads();
-    for (unsigned long long k = 2; k <= (unsigned long long)tile; k <<= 1) tile_stages(s, tile, 0ull, k, (int)(k >> 1));
+    for (unsigned long long k = 2; k <= (unsigned long long)tile2; k <<= 1) tile_stages(s, tile2, 0ull, k, (int)(k >> 1));
     for (int i = threadIdx.x; i < S; i += blockDim.x) {
         states_out[i] = s[i].q;
         energies_out[i] = f64_from_key(s[i].key);

@@ -14,13 +14,20 @@
 
 namespace ising {
 
-__global__ void __launch_bounds__(256) stage_kernel(const double* __restrict__ J, const double* __restrict__ h, int N,
+constexpr int STAGE_THREADS = 1024;
+
+__device__ void build_tables(Tables* __restrict__ tab, Ctrl* __restrict__ ctrl, int N);
+
+__global__ void __launch_bounds__(STAGE_THREADS) stage_kernel(const double* __restrict__ J, const double* __restrict__ h, int N,
                                                     Tables* __restrict__ tab, Ctrl* __restrict__ ctrl,
-                                                    double extra_eps_rel)
+                                                    unsigned* __restrict__ hist, double extra_eps_rel)
 {
+    // the candidate histogram of the call starts empty (walk.cuh)
+    if (hist)
+        for (int i = threadIdx.x; i < HIST_WORDS / 4; i += blockDim.x) reinterpret_cast<uint4*>(hist)[i] = make_uint4(0u, 0u, 0u, 0u);
     __shared__ int s_status;
     __shared__ int s_p;
-    __shared__ double s_red[256];
+    __shared__ double s_red[STAGE_THREADS];
     const int tid = threadIdx.x;
     constexpr int NO_ERROR_YET = -1000;
     if (tid == 0) s_status = NO_ERROR_YET;
@@ -54,7 +61,7 @@ __global__ void __launch_bounds__(256) stage_kernel(const double* __restrict__ J
     for (int i = tid; i < N; i += blockDim.x) part += fabs(h[i]);
     s_red[tid] = part;
     __syncthreads();
-    for (int s = 128; s > 0; s >>= 1) {
+    for (int s = STAGE_THREADS / 2; s > 0; s >>= 1) {
         if (tid < s) s_red[tid] += s_red[tid + s];
         __syncthreads();
     }
@@ -69,10 +76,11 @@ __global__ void __launch_bounds__(256) stage_kernel(const double* __restrict__ J
         for (int idx = tid; idx < N * N + N; idx += blockDim.x) {
             const double v = idx < N * N ? J[idx] : h[idx - N * N];
             if (v != 0.0 && isfinite(v)) {
-                int e;
-                const double m = frexp(fabs(v), &e);
-                const unsigned long long M = (unsigned long long)ldexp(m, 53);
-                const int low = e - 53 + (__ffsll((long long)M) - 1);
+                // |v| = M 2^base with the integer M read straight from the bit pattern (normal: implicit leading one)
+                const unsigned long long bits = (unsigned long long)__double_as_longlong(fabs(v));
+                const int eb = (int)(bits >> 52);
+                const unsigned long long M = (bits & 0xfffffffffffffull) | (eb ? 0x10000000000000ull : 0ull);
+                const int low = (eb ? eb - 1075 : -1074) + (__ffsll((long long)M) - 1);
                 if (-low > req) req = -low;
             }
         }
@@ -104,14 +112,17 @@ __global__ void __launch_bounds__(256) stage_kernel(const double* __restrict__ J
     __syncthreads();
     unsigned long long wq = 0ull;
     double err = 0.0;
+    // x 2^p and x 2^-p as exact multiplications (|p| <= 1000: both powers are normal doubles)
+    const double scale = __longlong_as_double((long long)(p + 1023) << 52);
+    const double inv_scale = __longlong_as_double((long long)(1023 - p) << 52);
     for (int idx = tid; idx < 64 * 64; idx += blockDim.x) {
         int i = idx >> 6, j = idx & 63;
         int q = 0;
         if (i < N && j < N && i != j) {
             double v = J[i * N + j];
-            double r = rint(ldexp(v, p));
+            double r = rint(v * scale);
             q = (int)r;
-            if (i < j) { err += fabs(ldexp(r, -p) - v); wq += (unsigned long long)(q < 0 ? -(long long)q : (long long)q); }
+            if (i < j) { err += fabs(r * inv_scale - v); wq += (unsigned long long)(q < 0 ? -(long long)q : (long long)q); }
         }
         tab->Jq[idx] = q;
     }
@@ -119,9 +130,9 @@ __global__ void __launch_bounds__(256) stage_kernel(const double* __restrict__ J
         int q = 0;
         if (i < N) {
             double v = FIELD_TERM_SIGN * h[i];                 // the one place the field sign convention enters the grid
-            double r = rint(ldexp(v, p));
+            double r = rint(v * scale);
             q = (int)r;
-            err += fabs(ldexp(r, -p) - v);
+            err += fabs(r * inv_scale - v);
             wq += (unsigned long long)(q < 0 ? -(long long)q : (long long)q);
         }
         tab->hq[i] = q;
@@ -129,7 +140,7 @@ __global__ void __launch_bounds__(256) stage_kernel(const double* __restrict__ J
     s_red[tid] = err;
     if (wq) atomicAdd(&s_wq, wq);
     __syncthreads();
-    for (int s = 128; s > 0; s >>= 1) {
+    for (int s = STAGE_THREADS / 2; s > 0; s >>= 1) {
         if (tid < s) s_red[tid] += s_red[tid + s];
         __syncthreads();
     }
@@ -169,12 +180,14 @@ __global__ void __launch_bounds__(256) stage_kernel(const double* __restrict__ J
         ctrl->hits = 0ull;
         ctrl->false_hits = 0ull;
     }
+    __syncthreads();                       // Jq, hq (global, written by this block) and Ctrl are complete
+    build_tables(tab, ctrl, N);
 }
 
-// Tables of the QUBO form relative to the base state (see file header). One block; thread-per-entry loops.
-__global__ void __launch_bounds__(256) tables_kernel(Tables* __restrict__ tab, Ctrl* __restrict__ ctrl, int N)
+// Tables of the QUBO form relative to the base state (see file header). Runs at the end of stage_kernel (one block);
+// thread-per-entry loops.
+__device__ void build_tables(Tables* __restrict__ tab, Ctrl* __restrict__ ctrl, int N)
 {
-    if (ctrl->status != ISING_OK) return;
     const int tid = threadIdx.x;
     const int* Jq = tab->Jq;
     auto Jat = [&](int i, int j) -> int { return (i < N && j < N) ? Jq[i * 64 + j] : 0; };
@@ -232,17 +245,30 @@ __global__ void __launch_bounds__(256) tables_kernel(Tables* __restrict__ tab, C
     //   cC = (BC >> s) + 2,  cU = (BU >> s) + 2 + LW_MAX,  bV = (BV >> s) + 2 + LW_MAX + cC   (register set b holds
     //   V + C[16][.], hence the extra cC);  the largest half a sum can reach is 2 (bV + cC + cU) <= 65535.
     __shared__ int s_shift, s_cC;
+    __shared__ unsigned long long s_BV, s_BU, s_BC;
+    if (tid == 0) { s_BV = 0ull; s_BU = 0ull; s_BC = 0ull; }
     __syncthreads();                                   // QL, QM, C above are complete
-    if (tid == 0) {
-        long long BV = 0, BU = 0, BC = 0, m;
-        for (int x = 0; x < NLO; ++x) { m = tab->QL[x]; m = m < 0 ? -m : m; if (m > BV) BV = m; }
-        for (int x = 0; x < NMID; ++x) { m = tab->QM[x]; m = m < 0 ? -m : m; if (m > BU) BU = m; }
-        for (int x = 0; x < NMID * NLO; ++x) { m = tab->C[x]; m = m < 0 ? -m : m; if (m > BC) BC = m; }
-        for (int i = 0; i < LOWBITS && i < N; ++i) {
-            long long R = tab->hq[i] < 0 ? -(long long)tab->hq[i] : tab->hq[i];
-            for (int j = 0; j < N; ++j) { m = Jq[i * 64 + j]; R += m < 0 ? -m : m; }
-            if (i < LL) BV += 2 * R; else BU += 2 * R;
+    {
+        unsigned long long m = 0ull;
+        for (int x = tid; x < NMID * NLO; x += blockDim.x) { const long long v = tab->C[x]; const unsigned long long a = (unsigned long long)(v < 0 ? -v : v); if (a > m) m = a; }
+        if (m) atomicMax(&s_BC, m);
+        if (tid < NLO) { const long long v = tab->QL[tid]; atomicMax(&s_BV, (unsigned long long)(v < 0 ? -v : v)); }
+        if (tid < NMID) { const long long v = tab->QM[tid]; atomicMax(&s_BU, (unsigned long long)(v < 0 ? -v : v)); }
+    }
+    __syncthreads();
+    // R_i = |hq_i| + sum_j |Jq_ij| for the ten low spins, one warp each
+    if (tid < 32 * LOWBITS) {
+        const int i = tid >> 5, lane = tid & 31;
+        unsigned long long R = 0ull;
+        if (i < N) {
+            for (int j = lane; j < N; j += 32) { const long long v = Jq[i * 64 + j]; R += (unsigned long long)(v < 0 ? -v : v); }
+            if (lane == 0) { const long long v = tab->hq[i]; R += (unsigned long long)(v < 0 ? -v : v); }
         }
+        if (R) atomicAdd(i < LL ? &s_BV : &s_BU, 2ull * R);
+    }
+    __syncthreads();
+    if (tid == 0) {
+        const long long BV = (long long)s_BV, BU = (long long)s_BU, BC = (long long)s_BC;
         int s = 0;
         long long cC = 0, cU = 0, bV = 0;
         for (; s < 40; ++s) {
@@ -292,11 +318,10 @@ __global__ void __launch_bounds__(256) tables_kernel(Tables* __restrict__ tab, C
     }
 }
 
-void launch_stage(const double* J, const double* h, int N, Tables* tab, Ctrl* ctrl, cudaStream_t st,
+void launch_stage(const double* J, const double* h, int N, Tables* tab, Ctrl* ctrl, unsigned* hist, cudaStream_t st,
                   double extra_eps_rel)
 {
-    stage_kernel<<<1, 256, 0, st>>>(J, h, N, tab, ctrl, extra_eps_rel);
-    tables_kernel<<<1, 256, 0, st>>>(tab, ctrl, N);
+    stage_kernel<<<1, STAGE_THREADS, 0, st>>>(J, h, N, tab, ctrl, hist, extra_eps_rel);
 }
 
 // QUBO -> Ising, eqs. (2),(3) inverted: J = a/4, h_i = b_i/2 + sum_j a_ij/4.

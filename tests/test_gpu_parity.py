@@ -799,3 +799,85 @@ def test_sharded_exchange_path_over_nccl_single_rank(B):
     finally:
         if created:
             dist.destroy_process_group()
+
+
+# ---------- the multi-rank path with the REAL C-ABI calls: two processes share the one GPU, gloo for the exchange ----------
+def _sharded_gpu_worker(rank, world, port, out_dir):
+    import torch
+    import torch.distributed as dist
+    from paper_1904_03621_b200 import binding as Bw, sharded
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    torch.cuda.set_device(0)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        c = I.baseline_config(3)
+        q, e = sharded.ising_lowest_sharded(c.J, c.h, c.S)          # binding.ising_lowest_range + ising_merge_lists
+        assert q.is_cuda and e.is_cuda
+        np.save(os.path.join(out_dir, f"q{rank}.npy"), Bw.states_to_numpy(q))
+        np.save(os.path.join(out_dir, f"e{rank}.npy"), e.cpu().numpy())
+        st = Bw.last_stats()
+        np.save(os.path.join(out_dir, f"n{rank}.npy"), np.array([st.kernel_launches]))
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("world", [2, 3])
+def test_sharded_two_processes_on_one_gpu(B, golden_dir, tmp_path, world):
+    """SURVEY.md 8(e) end to end: every rank enumerates its own range of cfg3 with the real kernels, the lists are
+    exchanged with one all-gather (gloo: NCCL refuses several ranks on one device) and merged by ising_merge_lists
+    on every rank. Every rank must end with the stored oracle list."""
+    import socket
+    import torch.multiprocessing as mp
+    s = socket.socket(); s.bind(("127.0.0.1", 0)); port = s.getsockname()[1]; s.close()
+    mp.spawn(_sharded_gpu_worker, args=(world, port, str(tmp_path)), nprocs=world, join=True)
+    c = I.baseline_config(3)
+    qo, eo = load_golden(os.path.join(golden_dir, "cfg3.txt"))
+    for r in range(world):
+        q = np.load(tmp_path / f"q{r}.npy"); e = np.load(tmp_path / f"e{r}.npy")
+        assert_exact(q, e, qo[:c.S], eo[:c.S])
+
+
+_FIRST_CALL_SCRIPT = r"""
+import sys, threading
+sys.path.insert(0, {root!r})
+import numpy as np, torch
+from paper_1904_03621_b200 import binding as B, instances as I
+B.load()
+ndev = torch.cuda.device_count()
+J, h = I.complete_gaussian(20, seed=7)
+S = 6000                                    # > 4096 kept entries: the multi-block sort with 64 KB of dynamic shared memory
+res = {{}}
+bar = threading.Barrier(2)
+def work(t):
+    torch.cuda.set_device(0)
+    bar.wait()                              # both threads make their FIRST library call at the same moment
+    q, e = B.ising_lowest(J, h, S)
+    res[t] = (B.states_to_numpy(q).tolist(), e.cpu().numpy().tolist())
+ths = [threading.Thread(target=work, args=(t,)) for t in range(2)]
+[t.start() for t in ths]; [t.join() for t in ths]
+assert res[0] == res[1] and len(res[0][0]) == S
+if ndev > 1:                                # one thread, two devices: the workspace and the attributes follow the device
+    for d in (0, 1, 0):
+        torch.cuda.set_device(d)
+        q, e = B.ising_lowest(torch.from_numpy(J).cuda(d), torch.from_numpy(h).cuda(d), S)
+        assert B.states_to_numpy(q).tolist() == res[0][0]
+np.save(sys.argv[1], np.array(res[0][0], dtype=np.uint64))
+print("ok", ndev)
+"""
+
+
+def test_first_calls_from_two_threads(B, tmp_path):
+    """include/ising.h: workspaces are per host thread and per device. A fresh process whose first two library calls
+    come from two threads at once (and, with a second device, from one thread on two devices); the sort needs the
+    per-device dynamic shared memory attribute."""
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    out = str(tmp_path / "q.npy")
+    r = subprocess.run([sys.executable, "-c", _FIRST_CALL_SCRIPT.format(root=root), out], capture_output=True, text=True,
+                       timeout=600)
+    assert r.returncode == 0, r.stderr[-2000:]
+    J, h = I.complete_gaussian(20, seed=7)
+    qo, _ = oracle.lowest(J, h, 6000)
+    assert np.load(out).tolist() == qo.tolist()
