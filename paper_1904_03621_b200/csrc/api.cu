@@ -28,6 +28,7 @@ struct Workspace {
     Entry* pool2 = nullptr;         // POOL_CAP entries: compacted candidates / band-pass scratch
     unsigned* hist = nullptr;       // HIST_WORDS counters: candidate histogram (walk.cuh)
     Tables* tab = nullptr;
+    ZTables* zt = nullptr;          // tables of the tensor-core screen
     Ctrl* ctrl = nullptr;
     Ctrl* h_ctrl = nullptr;         // pinned
     double* J2 = nullptr;           // 64*64 converted / staged couplings
@@ -37,11 +38,11 @@ struct Workspace {
     cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
     void release()
     {
-        cudaFree(pool); cudaFree(pool2); cudaFree(hist); cudaFree(tab); cudaFree(ctrl); cudaFree(J2); cudaFree(h2);
+        cudaFree(pool); cudaFree(pool2); cudaFree(hist); cudaFree(tab); cudaFree(zt); cudaFree(ctrl); cudaFree(J2); cudaFree(h2);
         cudaFree(out_q); cudaFree(out_e);
         if (h_ctrl) cudaFreeHost(h_ctrl);
         for (auto& e : ev) if (e) cudaEventDestroy(e);
-        pool = pool2 = nullptr; hist = nullptr; tab = nullptr; ctrl = h_ctrl = nullptr; J2 = h2 = nullptr;
+        pool = pool2 = nullptr; hist = nullptr; tab = nullptr; zt = nullptr; ctrl = h_ctrl = nullptr; J2 = h2 = nullptr;
         out_q = nullptr; out_e = nullptr;
         for (auto& e : ev) e = nullptr;
         device = -1;
@@ -75,6 +76,7 @@ int allocate_workspace(Workspace& ws, int dev)
     CUDA_TRY(cudaMalloc(&ws.pool2, sizeof(Entry) * (size_t)POOL_CAP));
     CUDA_TRY(cudaMalloc(&ws.hist, sizeof(unsigned) * (size_t)HIST_WORDS));
     CUDA_TRY(cudaMalloc(&ws.tab, sizeof(Tables)));
+    CUDA_TRY(cudaMalloc(&ws.zt, sizeof(ZTables)));
     CUDA_TRY(cudaMalloc(&ws.ctrl, sizeof(Ctrl)));
     CUDA_TRY(cudaMallocHost(&ws.h_ctrl, sizeof(Ctrl)));
     CUDA_TRY(cudaMalloc(&ws.J2, sizeof(double) * 64 * 64));
@@ -84,6 +86,7 @@ int allocate_workspace(Workspace& ws, int dev)
     for (auto& e : ws.ev) CUDA_TRY(cudaEventCreate(&e));
     (void)dev;
     set_select_attributes();                       // per-device function attributes (dynamic shared memory)
+    set_zscreen_attributes();
     CUDA_TRY(cudaGetLastError());
     return ISING_OK;
 }
@@ -118,8 +121,7 @@ int env_int(const char* name, int dflt, int lo, int hi)
 // host-sequenced path: between launches
 __global__ void reset_queue_kernel(Ctrl* ctrl, int drop_new)
 {
-    ctrl->next_unit = 0ull;
-    ctrl->done_configs = 0ull;
+    ctrl->next_unit = 0ull;                 // done_configs keeps counting: Segment::need_done is relative to q_begin
     if (drop_new) { ctrl->count = ctrl->kept; ctrl->pool_overflow = 0u; }
 }
 // restart of a whole run (after a void single-pass attempt) or start of the band pass
@@ -158,7 +160,7 @@ struct Run {
     Workspace* ws;
     ising_stats* stats;
     const double *J, *h, *Jorig, *horig;
-    int mode, N, S, variant, lw_max, chunk_log2, growth, qshift;
+    int mode, N, S, variant, lw_max, chunk_log2, growth, qshift, z_min_log2;
     unsigned keep_cap;
     unsigned long long q_begin, q_end;
     cudaStream_t st;
@@ -197,9 +199,9 @@ int launch_walk(const Run& r, const Plan& plan)
 {
     Workspace& ws = *r.ws;
     if (plan.total_units > 0x7fffffffull * WALK_WARPS) { t_last_error = "internal: too many units in one launch"; return ISING_ERR_INTERNAL; }
-    if (r.variant == 16) launch_walk16(ws.tab, ws.ctrl, ws.pool, ws.hist, plan, r.st);
+    if (r.variant != 32) launch_walk16(ws.tab, ws.ctrl, ws.pool, ws.hist, plan, r.st);
     else launch_walk32(ws.tab, ws.ctrl, ws.pool, ws.hist, plan, r.st);
-    LAUNCH_CHECK(r.variant == 16 ? "walk_kernel<Inner16>" : "walk_kernel<Inner32>");
+    LAUNCH_CHECK(r.variant != 32 ? "walk_kernel<Inner16>" : "walk_kernel<Inner32>");
     r.stats->kernel_launches += 1;
     r.stats->enum_launches += 1;
     return ISING_OK;
@@ -212,9 +214,80 @@ int read_ctrl(const Run& r)
     return ISING_OK;
 }
 
-// ---- single-pass path: ONE launch of the persistent kernel over the whole range (ramp-up segments, threshold
-// refreshed on the device), then compaction and the one-block final selection; one host synchronisation at the end.
-// Returns ISING_OK with *redo = true if the candidate pool overflowed (the run is void). ----
+// Segments of walked units for the states [cur, to): doubling while `doubling`, then (if `to` is the end of the range)
+// a last segment that takes all the rest and tapers its unit size so that the tail stays short.
+int plan_walk_segments(const Run& r, Plan& plan, int& ns, unsigned long long& cur, unsigned long long& units,
+                       unsigned long long to, unsigned long long need_floor)
+{
+    auto add_segment = [&](unsigned long long sz, int unit_bits, unsigned long long need) {
+        const unsigned long long nu = sz >> unit_bits;
+        plan.seg[ns] = Segment{cur, units, nu, need, unit_bits, 0};
+        units += nu;
+        cur += nu << unit_bits;
+        ++ns;
+    };
+    while (cur < to) {
+        const unsigned long long processed = cur - r.q_begin, remaining = to - cur;
+        const unsigned long long need = processed / 2 > need_floor ? processed / 2 : need_floor;
+        const unsigned long long target = (unsigned long long)r.growth * processed;
+        if (ns >= MAX_SEGMENTS - 12) { t_last_error = "internal: bad work plan"; return ISING_ERR_INTERNAL; }
+        if (target < remaining && target < (1ull << r.chunk_log2)) {
+            const int Lw = choose_lw(cur, target, r.lw_max);
+            add_segment(target, MIN_CHUNK_BITS + Lw, need);
+            continue;
+        }
+        // last segment(s): 7/8 of what is left at the full walk length, then 7/8 of the rest with 8x shorter units, ...
+        int Lw = choose_lw(cur, remaining, r.lw_max);
+        while (cur < to) {
+            const unsigned long long left = to - cur;
+            while (Lw > 0 && (cur & ((1ull << (MIN_CHUNK_BITS + Lw)) - 1ull))) --Lw;         // alignment of cur
+            unsigned long long sz = left;                                                  // Lw = 0: all of it
+            if (Lw > 0) sz = (left - (left >> 3)) >> (MIN_CHUNK_BITS + Lw) << (MIN_CHUNK_BITS + Lw);
+            if (sz >> (MIN_CHUNK_BITS + Lw)) {
+                if (ns >= MAX_SEGMENTS) { t_last_error = "internal: bad work plan"; return ISING_ERR_INTERNAL; }
+                add_segment(sz, MIN_CHUNK_BITS + Lw, need);
+            }
+            Lw = Lw > 3 ? Lw - 3 : 0;
+        }
+    }
+    return ISING_OK;
+}
+
+// Segments of tensor-core-screen units (2^(21 + Lw) configurations, one CTA each) for [cur, to), tapered at the end.
+int plan_z_segments(const Run& r, Plan& plan, int& ns, unsigned long long& cur, unsigned long long& units,
+                    unsigned long long to, bool taper)
+{
+    const int zu = ZB + 7;                                              // unit bits at Lw = 0
+    int Lw = floor_log2(to - cur) - zu - 10;                            // about 2^10 units: a few waves of CTAs
+    Lw = Lw < 0 ? 0 : (Lw > r.lw_max ? r.lw_max : Lw);
+    while (cur < to) {
+        const unsigned long long left = to - cur;
+        while (Lw > 0 && (cur & ((1ull << (zu + Lw)) - 1ull))) --Lw;
+        unsigned long long sz = left;
+        if (Lw > 0 && taper) sz = (left - (left >> 3)) >> (zu + Lw) << (zu + Lw);
+        const unsigned long long nu = sz >> (zu + Lw);
+        if (nu) {
+            if (ns >= MAX_SEGMENTS) { t_last_error = "internal: bad work plan"; return ISING_ERR_INTERNAL; }
+            plan.seg[ns] = Segment{cur, units, nu, 0ull, zu + Lw, 0};
+            units += nu;
+            cur += nu << (zu + Lw);
+            ++ns;
+        } else if (Lw == 0) {
+            t_last_error = "internal: range not aligned for the tensor-core screen";
+            return ISING_ERR_INTERNAL;
+        }
+        Lw = Lw > 3 ? Lw - 3 : 0;
+    }
+    return ISING_OK;
+}
+
+// ---- single-pass path: the whole range in one to three launches without host decisions in between (except the
+// one described below), threshold refreshed on the device, then compaction and the one-block final selection.
+// Ranges of 2^z_min_log2 states and more: the bulk goes through the tensor-core screen (zscreen.cu) -- the packed
+// kernel ramps the threshold up over the first 2^34 states (or an eighth of the range), the next stretch of the same
+// size is a PROBE of the screen, and only if fewer than 1 in 128 of its blocks were flagged (an instance whose table
+// range forces a blunt lambda, or a spectrum dense at the bottom, fails this) does the rest follow the same way;
+// otherwise the packed kernel finishes. Returns ISING_OK with *redo = true if the candidate pool overflowed. ----
 int run_single_pass(Run& r, unsigned long long* states_out, double* energies_out, bool* redo)
 {
     Workspace& ws = *r.ws;
@@ -223,73 +296,121 @@ int run_single_pass(Run& r, unsigned long long* states_out, double* energies_out
     plan_header(r, plan, 1, INT32_MIN);
     const unsigned long long range = r.q_end - r.q_begin;
     const bool direct = r.N <= N_DIRECT_MAX;
-    CUDA_TRY(cudaEventRecord(ws.ev[2], r.st));
+    const bool use_z = !direct && (r.variant == 0 || r.variant == 128) && range >= (1ull << r.z_min_log2) &&
+                       range >= (1ull << (ZB + 7 + 3)) && (r.q_begin & ((1ull << (ZB + 7)) - 1ull)) == 0;
+    int rc = ISING_OK;
+    auto timed_launch = [&](auto&& launch) -> int {
+        CUDA_TRY(cudaEventRecord(ws.ev[2], r.st));
+        const int lrc = launch();
+        if (lrc != ISING_OK) return lrc;
+        CUDA_TRY(cudaEventRecord(ws.ev[3], r.st));
+        return ISING_OK;
+    };
+    auto add_elapsed = [&]() -> int {
+        float ms = 0.f;
+        CUDA_TRY(cudaEventElapsedTime(&ms, ws.ev[2], ws.ev[3]));
+        r.enum_ms += ms;
+        return ISING_OK;
+    };
     if (direct) {
-        launch_direct(ws.tab, ws.ctrl, ws.pool, ws.hist, r.N, r.S, (unsigned)range, 1, r.st);
-        LAUNCH_CHECK("direct_kernel");
-        r.stats->kernel_launches += 1;
-        r.stats->enum_launches += 1;
+        rc = timed_launch([&]() -> int {
+            launch_direct(ws.tab, ws.ctrl, ws.pool, ws.hist, r.N, r.S, (unsigned)range, 1, r.st);
+            LAUNCH_CHECK("direct_kernel");
+            r.stats->kernel_launches += 1;
+            r.stats->enum_launches += 1;
+            return ISING_OK;
+        });
+        if (rc != ISING_OK) return rc;
     } else {
         // a2': the first X states are formed exactly, one 1024-configuration block per warp -- 2^15 of them without any
         // threshold, the rest under the threshold those give (which most blocks would pass anyway; X shrinks with S so
-        // that the candidates of this phase, about X S / 2^15, stay far below the pool size). Then walked segments
-        // that double; the last segment takes all the rest and tapers its unit size so that the tail stays short.
+        // that the candidates of this phase, about X S / 2^15, stay far below the pool size). Then walked segments.
         const unsigned long long prime = 1ull << MIN_CHUNK_BITS;
         unsigned long long X = 1ull << 21;
         while (X > prime && X * (unsigned long long)r.S > (1ull << 35)) X >>= 1;
         if (X > range) X = range;
+        unsigned long long p0 = range;                                   // end of the packed kernel's stretch
+        if (use_z) { p0 = 1ull << 34; while (p0 > range / 8) p0 >>= 1; }
         int ns = 0;
         unsigned long long cur = r.q_begin, units = 0;
-        auto add_segment = [&](unsigned long long sz, int unit_bits, unsigned long long need) {
-            const unsigned long long nu = sz >> unit_bits;
-            plan.seg[ns] = Segment{cur, units, nu, need, unit_bits, 0};
-            units += nu;
-            cur += nu << unit_bits;
-            ++ns;
-        };
-        add_segment(prime, LOWBITS, 0ull);
-        if (X > prime) add_segment(X - prime, LOWBITS, prime);
-        while (cur < r.q_end) {
-            const unsigned long long processed = cur - r.q_begin, remaining = r.q_end - cur;
-            const unsigned long long need = processed / 2 > prime ? processed / 2 : prime;
-            unsigned long long target = (unsigned long long)r.growth * processed;
-            if (ns >= MAX_SEGMENTS - 12) { t_last_error = "internal: bad work plan"; return ISING_ERR_INTERNAL; }
-            if (target < remaining && target < (1ull << r.chunk_log2)) {
-                const int Lw = choose_lw(cur, target, r.lw_max);
-                add_segment(target, MIN_CHUNK_BITS + Lw, need);
-                continue;
-            }
-            // last segment(s): 7/8 of what is left at the full walk length, then 7/8 of the rest with 8x shorter units, ...
-            int Lw = choose_lw(cur, remaining, r.lw_max);
-            while (cur < r.q_end) {
-                const unsigned long long left = r.q_end - cur;
-                while (Lw > 0 && (cur & ((1ull << (MIN_CHUNK_BITS + Lw)) - 1ull))) --Lw;         // alignment of cur
-                unsigned long long sz = left;                                                  // Lw = 0: all of it
-                if (Lw > 0) sz = (left - (left >> 3)) >> (MIN_CHUNK_BITS + Lw) << (MIN_CHUNK_BITS + Lw);
-                if (sz >> (MIN_CHUNK_BITS + Lw)) {
-                    if (ns >= MAX_SEGMENTS) { t_last_error = "internal: bad work plan"; return ISING_ERR_INTERNAL; }
-                    add_segment(sz, MIN_CHUNK_BITS + Lw, need);
-                }
-                Lw = Lw > 3 ? Lw - 3 : 0;
-            }
+        plan.seg[ns++] = Segment{cur, units, prime >> LOWBITS, 0ull, LOWBITS, 0};
+        units += prime >> LOWBITS; cur += prime;
+        if (X > prime) {
+            plan.seg[ns++] = Segment{cur, units, (X - prime) >> LOWBITS, prime, LOWBITS, 0};
+            units += (X - prime) >> LOWBITS; cur += X - prime;
         }
+        rc = plan_walk_segments(r, plan, ns, cur, units, r.q_begin + p0, prime);
+        if (rc != ISING_OK) return rc;
         plan.nseg = ns;
         plan.total_units = units;
-        int rc = launch_walk(r, plan);
+        rc = timed_launch([&]() -> int { return launch_walk(r, plan); });
         if (rc != ISING_OK) return rc;
+        if (use_z) {
+            launch_ztables(ws.tab, ws.ctrl, ws.zt, r.N, r.st);
+            LAUNCH_CHECK("ztables_kernel");
+            // ---- probe: the next p0 states through the tensor-core screen ----
+            reset_queue_kernel<<<1, 1, 0, r.st>>>(ws.ctrl, 0);
+            Plan zp;
+            plan_header(r, zp, 1, INT32_MIN);
+            ns = 0; units = 0;
+            rc = plan_z_segments(r, zp, ns, cur, units, r.q_begin + 2 * p0, false);
+            if (rc != ISING_OK) return rc;
+            zp.nseg = ns; zp.total_units = units;
+            CUDA_TRY(cudaEventRecord(ws.ev[3], r.st));                   // (the ramp-up launch ends here)
+            rc = read_ctrl(r);                                           // ... and is timed while the probe is enqueued
+            if (rc != ISING_OK) return rc;
+            if ((rc = add_elapsed()) != ISING_OK) return rc;
+            if (ws.h_ctrl->status != ISING_OK) return ISING_OK;
+            rc = timed_launch([&]() -> int {
+                launch_zwalk(ws.tab, ws.zt, ws.ctrl, ws.pool, ws.hist, zp, r.st);
+                LAUNCH_CHECK("zwalk_kernel");
+                return ISING_OK;
+            });
+            if (rc != ISING_OK) return rc;
+            r.stats->kernel_launches += 3;
+            r.stats->enum_launches += 1;
+            rc = read_ctrl(r);
+            if (rc != ISING_OK) return rc;
+            if ((rc = add_elapsed()) != ISING_OK) return rc;
+            const double zs = (double)ws.h_ctrl->z_steps, zf = (double)ws.h_ctrl->z_flagged;
+            const bool z_ok = !ws.h_ctrl->pool_overflow && zs > 0.0 && zf * 128.0 <= zs;
+            reset_queue_kernel<<<1, 1, 0, r.st>>>(ws.ctrl, 0);
+            r.stats->kernel_launches += 1;
+            Plan rest;
+            plan_header(r, rest, 1, INT32_MIN);
+            ns = 0; units = 0;
+            if (z_ok) {
+                rc = plan_z_segments(r, rest, ns, cur, units, r.q_end, true);
+                r.stats->kernel_variant = 128;
+            } else {
+                rc = plan_walk_segments(r, rest, ns, cur, units, r.q_end, 0ull);
+            }
+            if (rc != ISING_OK) return rc;
+            rest.nseg = ns; rest.total_units = units;
+            if (cur != r.q_end) { t_last_error = "internal: work plan does not cover the range"; return ISING_ERR_INTERNAL; }
+            rc = timed_launch([&]() -> int {
+                if (!z_ok) return launch_walk(r, rest);
+                launch_zwalk(ws.tab, ws.zt, ws.ctrl, ws.pool, ws.hist, rest, r.st);
+                LAUNCH_CHECK("zwalk_kernel");
+                r.stats->kernel_launches += 1;
+                r.stats->enum_launches += 1;
+                return ISING_OK;
+            });
+            if (rc != ISING_OK) return rc;
+        } else if (cur != r.q_end) {
+            t_last_error = "internal: work plan does not cover the range";
+            return ISING_ERR_INTERNAL;
+        }
     }
-    CUDA_TRY(cudaEventRecord(ws.ev[3], r.st));
     r.stats->kernel_launches += launch_compact(ws.pool, ws.pool2, ws.ctrl, plan, r.st);
     LAUNCH_CHECK("compact_kernel");
     r.stats->kernel_launches += launch_final_small(r.mode ? r.Jorig : r.J, r.mode ? r.horig : r.h, r.N, r.mode, ws.pool2,
                                                    ws.ctrl, r.S, r.keep_cap, states_out, energies_out, r.st);
     LAUNCH_CHECK("final_small_kernel");
     CUDA_TRY(cudaEventRecord(ws.ev[1], r.st));          // end of the call if the one-block selection sufficed
-    int rc = read_ctrl(r);
+    rc = read_ctrl(r);
     if (rc != ISING_OK) return rc;
-    float ms = 0.f;
-    CUDA_TRY(cudaEventElapsedTime(&ms, ws.ev[2], ws.ev[3]));
-    r.enum_ms += ms;
+    if ((rc = add_elapsed()) != ISING_OK) return rc;
     const Ctrl& c = *ws.h_ctrl;
     if (c.status != ISING_OK) return ISING_OK;          // rejected by the staging kernel: the caller reports it
     r.stats->configs += range;
@@ -439,7 +560,11 @@ int run_lowest(const double* J, const double* h, const double* Jorig, const doub
     r.lw_max = env_int("ISING_LW", LW_MAX, 0, LW_MAX);
     r.chunk_log2 = env_int("ISING_CHUNK_LOG2", 42, MIN_CHUNK_BITS, 44);
     r.growth = env_int("ISING_GROWTH", 3, 1, 1 << 20);      // a segment is at most growth x what lies before it
-    r.variant = env_int("ISING_KERNEL", 16, 16, 32) == 32 ? 32 : 16;   // 16: packed screen, 32: int32 kernel
+    // 0 (default): packed 16-bit screen, plus the tensor-core screen for the bulk of large ranges; 16: packed screen only;
+    // 32: int32 kernel only; 128: as 0
+    const int kv = env_int("ISING_KERNEL", 0, 0, 128);
+    r.variant = kv == 32 ? 32 : (kv == 16 ? 16 : 0);
+    r.z_min_log2 = env_int("ISING_Z_MIN_LOG2", 37, ZB + 10, 63);
     // test knob for the band pass: a selection keeps at most 2^k entries (never fewer than S)
     r.keep_cap = 1u << env_int("ISING_KEEP_CAP_LOG2", 20, 5, 20);
     while (r.keep_cap < (unsigned)S) r.keep_cap <<= 1;
@@ -453,7 +578,7 @@ int run_lowest(const double* J, const double* h, const double* Jorig, const doub
     LAUNCH_CHECK("stage_kernel");
     stats.kernel_launches += 1;
     stats.inner_bits = LOWBITS;
-    stats.kernel_variant = r.variant;
+    stats.kernel_variant = r.variant == 32 ? 32 : 16;      // 128 once the tensor-core screen took the bulk
     stats.passes = 1;
 
     bool redo = (path == 1);
@@ -472,7 +597,7 @@ int run_lowest(const double* J, const double* h, const double* Jorig, const doub
     stats.grid_exponent = ws.h_ctrl->p;
     stats.exact = ws.h_ctrl->exact;
     stats.epsilon = ws.h_ctrl->epsilon;
-    stats.screen_shift = r.variant == 16 ? ws.h_ctrl->shift16 : -1;
+    stats.screen_shift = r.variant != 32 ? ws.h_ctrl->shift16 : -1;
     const int band = ws.h_ctrl->band;
 
     if (redo) {

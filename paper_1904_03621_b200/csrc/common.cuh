@@ -116,6 +116,8 @@ struct Ctrl {
     unsigned pad0;
     unsigned long long hits;   // 1024-configuration blocks that passed the screen and were formed exactly
     unsigned long long false_hits;     // ... of which none passed the exact test
+    unsigned long long z_steps;        // tensor-core screen (zscreen.cu): 2^14-configuration blocks screened
+    unsigned long long z_flagged;      // ... of which flagged (formed exactly as 16 blocks of 1024)
 };
 
 // Instance tables in grid units, built once per call by build_tables (stage.cu).
@@ -137,6 +139,18 @@ struct Tables {
     unsigned Cp[(NMID / 2) * NLO]; // Cp[u][lo]  = pack( (C[m0][lo] >> s) + cC , (C[m0 | 8][lo] >> s) + cC ),  m0 = (u & 7) | ((u >> 3) << 4)
     unsigned DVp[LW_MAX * 2 * NLO];        // DVp[k][sb][lo] = +-(DV[k][1][lo] >> s) * 65537    (both halves alike)
     unsigned DUp[LW_MAX * 2 * (NMID / 2)]; // DUp[k][sb][u]  = +-((DU[k][1][m0] >> s) + 65536 (DU[k][1][m0 | 8] >> s))
+};
+
+// Tables of the tensor-core screen (zscreen.cu), built once per call by ztables_kernel.
+constexpr int ZB = 14;                 // block bits of the screen: lo = spins 0..6 (K), mid = spins 7..13 (N)
+struct ZTables {
+    uint4 Tb[2048];                    // bf16 T[mid][lo] = 2^(-lambda C'(lo,mid) + t0) in the UMMA canonical K-major layout
+    int DPhi[LW_MAX * 16];             // DPhi[k][i] = 2 Jq[i][ZB + k]: change of Phi_i when walk bit k turns on
+    int DWz[1 << LW_MAX];              // walk-internal part of Gray step t for walk spins ZB + k (cf. Tables::DW)
+    int Cz[1 << ZB];                   // C'(lo | mid << 7) = -4 sum_{a<b set} Jq_ab, grid units
+    float lambda;                      // bits per grid unit
+    float t0;                          // centres log2 T in [-THETA, +THETA]
+    int cmin, cmax;
 };
 
 // One segment of the work plan: n_units units of 2^unit_bits configurations starting at state q0.
@@ -175,6 +189,11 @@ void launch_walk32(const Tables* tab, Ctrl* ctrl, Entry* pool, unsigned* hist, c
 void launch_walk16(const Tables* tab, Ctrl* ctrl, Entry* pool, unsigned* hist, const Plan& plan, cudaStream_t st);
 void launch_direct(const Tables* tab, Ctrl* ctrl, Entry* pool, unsigned* hist, int N, int S, unsigned count,
                    int use_hist, cudaStream_t st);
+// zscreen.cu: the tensor-core (tcgen05) screen
+void launch_ztables(const Tables* tab, const Ctrl* ctrl, ZTables* zt, int N, cudaStream_t st);
+void launch_zwalk(const Tables* tab, const ZTables* zt, Ctrl* ctrl, Entry* pool, unsigned* hist, const Plan& plan,
+                  cudaStream_t st);
+void set_zscreen_attributes();
 // select.cu
 int  launch_select(Entry* pool, Ctrl* ctrl, unsigned n, int S, const Plan& plan, cudaStream_t st);   // returns kernels launched
 int  launch_compact(const Entry* pool, Entry* pool2, Ctrl* ctrl, const Plan& plan, cudaStream_t st);

@@ -179,6 +179,8 @@ __global__ void __launch_bounds__(STAGE_THREADS) stage_kernel(const double* __re
         ctrl->blocks_done = 0;
         ctrl->hits = 0ull;
         ctrl->false_hits = 0ull;
+        ctrl->z_steps = 0ull;
+        ctrl->z_flagged = 0ull;
     }
     __syncthreads();                       // Jq, hq (global, written by this block) and Ctrl are complete
     build_tables(tab, ctrl, N);
