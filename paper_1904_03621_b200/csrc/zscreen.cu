@@ -57,6 +57,11 @@ __device__ __forceinline__ unsigned long long umma_desc(unsigned saddr)
 
 __device__ __forceinline__ float ex2f(float x) { float r; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
 __device__ __forceinline__ float lg2f(float x) { float r; asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+// packed fp32 pairs (FMUL2 / FFMA2): two lanes per issue slot
+__device__ __forceinline__ unsigned long long pk2(float lo, float hi) { unsigned long long r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
+__device__ __forceinline__ void upk2(unsigned long long v, float& lo, float& hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ unsigned long long mul2(unsigned long long a, unsigned long long b) { unsigned long long r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ unsigned long long fma2(unsigned long long a, unsigned long long b, unsigned long long c) { unsigned long long r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
 __device__ __forceinline__ unsigned pack_bf16(float lo, float hi)
 {
     unsigned r;
@@ -141,13 +146,13 @@ zwalk_kernel(const Tables* __restrict__ tab, const ZTables* __restrict__ zt, Ctr
     extern __shared__ __align__(1024) unsigned char zsmem[];
     unsigned char* sT = zsmem;                       // 32 KB: B operand (the instance table)
     unsigned char* sA = zsmem + 32768;               // 32 KB: A operand (one row per thread)
-    __shared__ __align__(8) unsigned long long mbar;
+    __shared__ __align__(8) unsigned long long mbar[1];
     __shared__ unsigned s_tmem;
     __shared__ unsigned long long s_unit;
     __shared__ int sDWz[1 << LW_MAX];
     __shared__ __align__(16) int sDPhi[LW_MAX * 16];
     __shared__ int sPhiW[LW_MAX][Z_THREADS];
-    __shared__ int sPhiB[Z_THREADS / 32][64];
+    int (*sPhiB)[64] = reinterpret_cast<int (*)[64]>(sA);   // base-state scratch: lives in the A tile until the first step
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     if (ctrl->status != 0) return;
@@ -157,7 +162,7 @@ zwalk_kernel(const Tables* __restrict__ tab, const ZTables* __restrict__ zt, Ctr
     for (int i = tid; i < (1 << LW_MAX); i += Z_THREADS) sDWz[i] = zt->DWz[i];
     for (int i = tid; i < LW_MAX * 16; i += Z_THREADS) sDPhi[i] = zt->DPhi[i];
     if (tid == 0) {
-        asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"(smem_u32(&mbar)), "r"(1));
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"(smem_u32(&mbar[0])), "r"(1));
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
@@ -223,123 +228,161 @@ zwalk_kernel(const Tables* __restrict__ tab, const ZTables* __restrict__ zt, Ctr
         }
 #pragma unroll
         for (int i = 0; i < LW_MAX; ++i) sPhiW[i][tid] = PhiW[i];
+        __syncthreads();                                 // the scratch in the A tile is dead from here on
 
         unsigned long long tau = ld_relaxed_u64(&ctrl->tau);
         int tauE = tau_energy(tau);
-        unsigned parity = 0;
         const float two_lambda = 2.f * lambda;
-        unsigned char* myrow = sA + (unsigned)(tid >> 3) * Z_SBO + (unsigned)(tid & 7) * 16u;
+        const unsigned rowoff = (unsigned)(tid >> 3) * Z_SBO + (unsigned)(tid & 7) * 16u;
         const unsigned nsteps = 1u << Lw;
 
-        for (unsigned t = 0; t < nsteps; ++t) {
-            // ---- per-spin factors: bit set multiplies the weight by 2^y, y = 2 lambda Phi; normalised so that the
-            //      larger of the two factors of a spin is exactly 1 ----
+        // Factors of one step from the fourteen local fields, and the thread's A row into buffer `buf`:
+        //   bit set multiplies the weight by 2^y, y = 2 lambda Phi; normalised so that the larger of the two factors of
+        //   a spin is exactly 1. a[lo] = product over the 7 lo spins, 128 values, bf16, canonical layout; products in
+        //   packed fp32 pairs (FMUL2): pair p of Q holds lo = 2p (low lane: spin 0 down) and 2p + 1 (spin 0 up).
+        // Returns the mid-spin factors (for the fold) and  sum_i max(y_i, 0) - t0  (the instance part of L).
+        auto gen_row = [&](int buf, const int (&Ph)[ZB], float (&m0)[7], float (&m1)[7], float& lpb) {
             float r0[ZB], r1[ZB];
-            float Lp = lambda * (float)(tauE - Eh) - t0;
+            float acc = -t0;
 #pragma unroll
             for (int i = 0; i < ZB; ++i) {
-                const float y = two_lambda * (float)Phi[i];
+                const float y = two_lambda * (float)Ph[i];
                 const float e = ex2f(-fabsf(y));
                 r1[i] = y >= 0.f ? 1.f : e;
                 r0[i] = y >= 0.f ? e : 1.f;
-                Lp += fmaxf(y, 0.f);
+                acc += fmaxf(y, 0.f);
             }
-            // ---- A row: a[lo] = prod over the 7 lo spins, 128 values, bf16, canonical layout ----
-            {
-                float P[32];
-                P[0] = r0[0]; P[1] = r1[0];
+            lpb = acc;
 #pragma unroll
-                for (int b = 1; b < 5; ++b) {
+            for (int i = 0; i < 7; ++i) { m0[i] = r0[7 + i]; m1[i] = r1[7 + i]; }
+            unsigned long long Q[16];
+            Q[0] = pk2(r0[0], r1[0]);
 #pragma unroll
-                    for (int j = (1 << b) - 1; j >= 0; --j) {
-                        const float v = P[j];
-                        P[j + (1 << b)] = v * r1[b];
-                        P[j] = v * r0[b];
-                    }
-                }
+            for (int b = 1; b < 5; ++b) {
+                const unsigned long long f0 = pk2(r0[b], r0[b]), f1 = pk2(r1[b], r1[b]);
 #pragma unroll
-                for (int c = 0; c < 4; ++c) {
-                    const float f = ((c & 1) ? r1[5] : r0[5]) * ((c & 2) ? r1[6] : r0[6]);
-#pragma unroll
-                    for (int g = 0; g < 4; ++g) {
-                        uint4 w;
-                        w.x = pack_bf16(P[8 * g + 0] * f, P[8 * g + 1] * f);
-                        w.y = pack_bf16(P[8 * g + 2] * f, P[8 * g + 3] * f);
-                        w.z = pack_bf16(P[8 * g + 4] * f, P[8 * g + 5] * f);
-                        w.w = pack_bf16(P[8 * g + 6] * f, P[8 * g + 7] * f);
-                        *reinterpret_cast<uint4*>(myrow + (unsigned)(4 * c + g) * Z_LBO) = w;   // k-chunk lo/8 = 4c + g
-                    }
+                for (int j = (1 << (b - 1)) - 1; j >= 0; --j) {
+                    const unsigned long long v = Q[j];
+                    Q[j + (1 << (b - 1))] = mul2(v, f1);
+                    Q[j] = mul2(v, f0);
                 }
             }
-            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            unsigned char* myrow = sA + (unsigned)buf * 32768u + rowoff;
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+                const float f = ((c & 1) ? r1[5] : r0[5]) * ((c & 2) ? r1[6] : r0[6]);
+                const unsigned long long F = pk2(f, f);
+#pragma unroll
+                for (int g = 0; g < 4; ++g) {
+                    float e0, e1, e2, e3, e4, e5, e6, e7;
+                    upk2(mul2(Q[4 * g + 0], F), e0, e1);
+                    upk2(mul2(Q[4 * g + 1], F), e2, e3);
+                    upk2(mul2(Q[4 * g + 2], F), e4, e5);
+                    upk2(mul2(Q[4 * g + 3], F), e6, e7);
+                    uint4 w;
+                    w.x = pack_bf16(e0, e1);
+                    w.y = pack_bf16(e2, e3);
+                    w.z = pack_bf16(e4, e5);
+                    w.w = pack_bf16(e6, e7);
+                    *reinterpret_cast<uint4*>(myrow + (unsigned)(4 * c + g) * Z_LBO) = w;   // k-chunk lo/8 = 4c + g
+                }
+            }
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");    // the row is read by the tensor core
+        };
+        // One elected thread: D[buf] = A[buf] x T^T, eight K = 16 slices, completion signalled on mbar[buf].
+        auto issue_mma = [&](int buf) {
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+            const unsigned a0 = smem_u32(sA) + (unsigned)buf * 32768u, b0 = smem_u32(sT);
+#pragma unroll
+            for (int ks = 0; ks < 8; ++ks) {
+                const unsigned long long da = umma_desc(a0 + (unsigned)ks * 2u * Z_LBO);
+                const unsigned long long db = umma_desc(b0 + (unsigned)ks * 2u * Z_LBO);
+                const unsigned acc = ks > 0 ? 1u : 0u;
+                asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+                             "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
+                             :: "r"(tmem + (unsigned)buf * 128u), "l"(da), "l"(db), "r"(Z_IDESC), "r"(acc) : "memory");
+            }
+            asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];"
+                         :: "r"(smem_u32(&mbar[buf])) : "memory");
+        };
+
+        // ---- one step: rows -> tensor core -> fold. Three CTAs share an SM (single A tile, single accumulator), so
+        //      the phases of one CTA overlap with the other two. (A software pipeline inside the CTA -- two A tiles,
+        //      two accumulators -- was measured and dropped: the larger footprint leaves two CTAs per SM, and with eight
+        //      warps per SM the dependent chains of the row generation and the fold are not hidden: 4.2e14 against
+        //      4.9e14 configurations/s.) ----
+        float m0[7], m1[7], lpb;
+        for (unsigned t = 0; t < nsteps; ++t) {
+            gen_row(0, Phi, m0, m1, lpb);
             asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-            __syncthreads();                 // every A row is written; every TMEM read of the previous step is done
-            if (tid == 0) {
-                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-                const unsigned a0 = smem_u32(sA), b0 = smem_u32(sT);
-#pragma unroll
-                for (int ks = 0; ks < 8; ++ks) {
-                    const unsigned long long da = umma_desc(a0 + (unsigned)ks * 2u * Z_LBO);
-                    const unsigned long long db = umma_desc(b0 + (unsigned)ks * 2u * Z_LBO);
-                    const unsigned acc = ks > 0 ? 1u : 0u;
-                    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
-                                 "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
-                                 :: "r"(tmem), "l"(da), "l"(db), "r"(Z_IDESC), "r"(acc) : "memory");
-                }
-                asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];"
-                             :: "r"(smem_u32(&mbar)) : "memory");
-            }
+            __syncthreads();       // every A row is written; every TMEM read of the previous step is done
+            if (tid == 0) issue_mma(0);
             // ---- while the tensor core works: the Gray step that follows this block (walk bit k = ctz(t + 1)) ----
             const unsigned tn = t + 1 < nsteps ? t + 1 : 1u;
             const int k = __ffs(tn) - 1;
             const int sb = ((tn ^ (tn >> 1)) >> k) & 1;
             const int EhNext = Eh + sDWz[tn] + (sb ? -2 : 2) * sPhiW[k][tid];
-            int dphi[16];
             {
                 const int4* dp = reinterpret_cast<const int4*>(sDPhi + k * 16);
 #pragma unroll
                 for (int x = 0; x < 4; ++x) {
                     const int4 d = dp[x];
-                    dphi[4 * x + 0] = d.x; dphi[4 * x + 1] = d.y; dphi[4 * x + 2] = d.z; dphi[4 * x + 3] = d.w;
+                    if (4 * x + 0 < ZB) Phi[4 * x + 0] += sb ? d.x : -d.x;
+                    if (4 * x + 1 < ZB) Phi[4 * x + 1] += sb ? d.y : -d.y;
+                    if (4 * x + 2 < ZB) Phi[4 * x + 2] += sb ? d.z : -d.z;
+                    if (4 * x + 3 < ZB) Phi[4 * x + 3] += sb ? d.w : -d.w;
                 }
             }
             // ---- wait for the accumulator, fold this thread's row: R = sum_mid u[mid] D[mid] ----
             asm volatile("{\n\t.reg .pred P1;\n\tZWAIT_%=:\n\t"
                          "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n\t"
-                         "@P1 bra ZDONE_%=;\n\tbra ZWAIT_%=;\n\tZDONE_%=:\n\t}" :: "r"(smem_u32(&mbar)), "r"(parity) : "memory");
-            parity ^= 1u;
+                         "@P1 bra ZDONE_%=;\n\tbra ZWAIT_%=;\n\tZDONE_%=:\n\t}"
+                         :: "r"(smem_u32(&mbar[0])), "r"(t & 1u) : "memory");
             __syncwarp();
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-            float part[4];
+            // the fold in packed pairs (FMUL2 / FFMA2): the stages of mid bits 1..6 combine whole pairs (columns 2p, 2p+1);
+            // mid bit 0 (spin 7), which sits inside a pair, comes last. All four loads are issued before the one wait so
+            // that the four chunk folds are independent chains.
+            unsigned v[4][32];
 #pragma unroll
             for (int c = 0; c < 4; ++c) {
-                unsigned v[32];
                 const unsigned taddr = tmem + ((unsigned)(warp * 32) << 16) + (unsigned)(c * 32);
                 asm volatile("tcgen05.ld.sync.aligned.32x32b.x32.b32 "
                              "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
                              "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
-                             : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
-                               "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]),
-                               "=r"(v[16]), "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]),
-                               "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+                             : "=r"(v[c][0]), "=r"(v[c][1]), "=r"(v[c][2]), "=r"(v[c][3]), "=r"(v[c][4]), "=r"(v[c][5]), "=r"(v[c][6]), "=r"(v[c][7]),
+                               "=r"(v[c][8]), "=r"(v[c][9]), "=r"(v[c][10]), "=r"(v[c][11]), "=r"(v[c][12]), "=r"(v[c][13]), "=r"(v[c][14]), "=r"(v[c][15]),
+                               "=r"(v[c][16]), "=r"(v[c][17]), "=r"(v[c][18]), "=r"(v[c][19]), "=r"(v[c][20]), "=r"(v[c][21]), "=r"(v[c][22]), "=r"(v[c][23]),
+                               "=r"(v[c][24]), "=r"(v[c][25]), "=r"(v[c][26]), "=r"(v[c][27]), "=r"(v[c][28]), "=r"(v[c][29]), "=r"(v[c][30]), "=r"(v[c][31])
                              : "r"(taddr) : "memory");
-                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-                float x[32];
+            }
+            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+            unsigned long long part[4];
+            unsigned long long g0[7], g1[7];
 #pragma unroll
-                for (int j = 0; j < 32; ++j) x[j] = __uint_as_float(v[j]);
-                // mid bits 0..4 = spins 7..11: five butterfly stages
+            for (int i = 1; i < 7; ++i) { g0[i] = pk2(m0[i], m0[i]); g1[i] = pk2(m1[i], m1[i]); }
 #pragma unroll
-                for (int b = 0; b < 5; ++b) {
+            for (int c = 0; c < 4; ++c) {
+                unsigned long long x[16];
 #pragma unroll
-                    for (int j = 0; j < 32; j += (2 << b)) x[j] = fmaf(x[j + (1 << b)], r1[7 + b], x[j] * r0[7 + b]);
+                for (int p = 0; p < 16; ++p) x[p] = pk2(__uint_as_float(v[c][2 * p]), __uint_as_float(v[c][2 * p + 1]));
+                // mid bits 1..4 = spins 8..11: pair p covers mid = 2p, 2p + 1; bit b of mid is bit b - 1 of p
+#pragma unroll
+                for (int b = 1; b < 5; ++b) {
+#pragma unroll
+                    for (int p = 0; p < 16; p += (1 << b)) x[p] = fma2(x[p + (1 << (b - 1))], g1[b], mul2(x[p], g0[b]));
                 }
                 part[c] = x[0];
             }
-            // mid bits 5, 6 = spins 12, 13
-            const float h0 = fmaf(part[1], r1[12], part[0] * r0[12]);
-            const float h1 = fmaf(part[3], r1[12], part[2] * r0[12]);
-            const float R = fmaf(h1, r1[13], h0 * r0[13]);
+            // mid bits 5, 6 = spins 12, 13 (still in pairs), then mid bit 0 = spin 7 (inside the pair)
+            const unsigned long long h0 = fma2(part[1], g1[5], mul2(part[0], g0[5]));
+            const unsigned long long h1 = fma2(part[3], g1[5], mul2(part[2], g0[5]));
+            const unsigned long long hh = fma2(h1, g1[6], mul2(h0, g0[6]));
+            float Rlo, Rhi;
+            upk2(hh, Rlo, Rhi);
+            const float R = fmaf(Rhi, m1[0], Rlo * m0[0]);
             // ---- a4: flag unless the block provably holds no configuration with E <= tauE ----
+            const float Lp = fmaf(lambda, (float)(tauE - Eh), lpb);
             const bool clear = (lg2f(R) + Lp < -Z_MARGIN) && (Lp <= Z_L_SAFE);
             unsigned hits = __ballot_sync(0xffffffffu, !clear);
             flagged += __popc(hits);
@@ -357,8 +400,6 @@ zwalk_kernel(const Tables* __restrict__ tab, const ZTables* __restrict__ zt, Ctr
             }
             // ---- move on to step t + 1 ----
             Eh = EhNext;
-#pragma unroll
-            for (int i = 0; i < ZB; ++i) Phi[i] += sb ? dphi[i] : -dphi[i];
             if ((t & 15u) == 15u) {
                 tau = ld_relaxed_u64(&ctrl->tau);
                 tauE = tau_energy(tau);
