@@ -160,7 +160,7 @@ struct Run {
     Workspace* ws;
     ising_stats* stats;
     const double *J, *h, *Jorig, *horig;
-    int mode, N, S, variant, lw_max, chunk_log2, growth, qshift, z_min_log2;
+    int mode, N, S, variant, lw_max, chunk_log2, growth, qshift, z_min_log2, z_ramp_log2;
     unsigned keep_cap;
     unsigned long long q_begin, q_end;
     cudaStream_t st;
@@ -254,17 +254,20 @@ int plan_walk_segments(const Run& r, Plan& plan, int& ns, unsigned long long& cu
 }
 
 // Segments of tensor-core-screen units (2^(21 + Lw) configurations, one CTA each) for [cur, to), tapered at the end.
+// A CTA costs about 20 us before its first step (table copy, tensor-memory allocation, base state) and 3 us per step,
+// so units shorter than 2^5 steps are avoided wherever the alignment of the range allows.
 int plan_z_segments(const Run& r, Plan& plan, int& ns, unsigned long long& cur, unsigned long long& units,
                     unsigned long long to, bool taper)
 {
     const int zu = ZB + 7;                                              // unit bits at Lw = 0
-    int Lw = floor_log2(to - cur) - zu - 10;                            // about 2^10 units: a few waves of CTAs
-    Lw = Lw < 0 ? 0 : (Lw > r.lw_max ? r.lw_max : Lw);
+    int Lw = floor_log2(to - cur) - zu - 11;                            // about 2^11 units: several waves of CTAs
+    const int lw_floor = r.lw_max < 5 ? r.lw_max : 5;
+    Lw = Lw < lw_floor ? lw_floor : (Lw > r.lw_max ? r.lw_max : Lw);
     while (cur < to) {
         const unsigned long long left = to - cur;
-        while (Lw > 0 && (cur & ((1ull << (zu + Lw)) - 1ull))) --Lw;
-        unsigned long long sz = left;
-        if (Lw > 0 && taper) sz = (left - (left >> 3)) >> (zu + Lw) << (zu + Lw);
+        while (Lw > 0 && ((cur & ((1ull << (zu + Lw)) - 1ull)) || (left >> (zu + Lw)) == 0)) --Lw;
+        unsigned long long sz = left >> (zu + Lw) << (zu + Lw);
+        if (Lw > lw_floor && taper) sz = (left - (left >> 3)) >> (zu + Lw) << (zu + Lw);
         const unsigned long long nu = sz >> (zu + Lw);
         if (nu) {
             if (ns >= MAX_SEGMENTS) { t_last_error = "internal: bad work plan"; return ISING_ERR_INTERNAL; }
@@ -276,7 +279,10 @@ int plan_z_segments(const Run& r, Plan& plan, int& ns, unsigned long long& cur, 
             t_last_error = "internal: range not aligned for the tensor-core screen";
             return ISING_ERR_INTERNAL;
         }
-        Lw = Lw > 3 ? Lw - 3 : 0;
+        if (cur < to) {
+            const int next = Lw > lw_floor + 3 ? Lw - 3 : lw_floor;
+            Lw = next < Lw ? next : (Lw > 0 ? Lw - 1 : 0);                 // below the floor only to finish a ragged end
+        }
     }
     return ISING_OK;
 }
@@ -330,7 +336,7 @@ int run_single_pass(Run& r, unsigned long long* states_out, double* energies_out
         while (X > prime && X * (unsigned long long)r.S > (1ull << 35)) X >>= 1;
         if (X > range) X = range;
         unsigned long long p0 = range;                                   // end of the packed kernel's stretch
-        if (use_z) { p0 = 1ull << 34; while (p0 > range / 8) p0 >>= 1; }
+        if (use_z) { p0 = 1ull << r.z_ramp_log2; while (p0 > range / 8) p0 >>= 1; }
         int ns = 0;
         unsigned long long cur = r.q_begin, units = 0;
         plan.seg[ns++] = Segment{cur, units, prime >> LOWBITS, 0ull, LOWBITS, 0};
@@ -564,7 +570,8 @@ int run_lowest(const double* J, const double* h, const double* Jorig, const doub
     // 32: int32 kernel only; 128: as 0
     const int kv = env_int("ISING_KERNEL", 0, 0, 128);
     r.variant = kv == 32 ? 32 : (kv == 16 ? 16 : 0);
-    r.z_min_log2 = env_int("ISING_Z_MIN_LOG2", 37, ZB + 10, 63);
+    r.z_min_log2 = env_int("ISING_Z_MIN_LOG2", 36, ZB + 10, 63);
+    r.z_ramp_log2 = env_int("ISING_Z_RAMP_LOG2", 34, ZB + 7, 44);
     // test knob for the band pass: a selection keeps at most 2^k entries (never fewer than S)
     r.keep_cap = 1u << env_int("ISING_KEEP_CAP_LOG2", 20, 5, 20);
     while (r.keep_cap < (unsigned)S) r.keep_cap <<= 1;
