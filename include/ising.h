@@ -14,13 +14,22 @@
  *
  * All work runs in hand-written sm_100a CUDA kernels enqueued on the caller's stream. There is
  * no CPU fallback: without a CUDA device every compute entry point returns ISING_ERR_CUDA.
+ * Every configuration of the requested range is screened against the running S-th best energy --
+ * in blocks of 2^14 by a bf16 tensor-core (tcgen05) partition-function bound for the bulk of ranges
+ * of 2^36 states and more, in blocks of 2^10 by a packed 16-bit lower bound otherwise -- and every
+ * block that passes a screen is formed exactly in 32-bit integers; both screens can only add work
+ * (false hits), never lose a state (DESIGN.md sections 6, 6b). Environment knobs (development /
+ * tests): ISING_KERNEL = 16 (packed screen only) | 32 (int32 add-min per configuration, no screen),
+ * ISING_Z_MIN_LOG2, ISING_Z_RAMP_LOG2, ISING_LW, ISING_CHUNK_LOG2, ISING_GROWTH, ISING_PATH = 1
+ * (host-sequenced pieces), ISING_KEEP_CAP_LOG2.
  *
  * Pointer arguments say in their name where they live: *_dev = device memory, *_host = host memory.
- * The library never frees or retains caller buffers. Scratch (a 32 MiB candidate pool, the instance
- * tables, a pinned control block) is allocated on first use per host thread and device, reused by that
- * thread's later calls, and released by ising_release_workspace().
- * Every compute entry point SYNCHRONISES the stream before it returns (the launch loop is host
- * sequenced), so outputs are valid on return. On any error the output buffers are left untouched
+ * The library never frees or retains caller buffers. Scratch (two 64 MiB candidate pools, a 257 KiB
+ * candidate histogram, the instance tables, a pinned control block) is allocated on first use per host
+ * thread and device, reused by that thread's later calls, and released by ising_release_workspace()
+ * or when the thread exits.
+ * Every compute entry point SYNCHRONISES the stream before it returns (normally once, at the end: the
+ * threshold is refreshed on the device), so outputs are valid on return. On any error the output buffers are left untouched
  * (device variants) or unspecified (host variants) and a negative ISING_ERR_* code is returned.
  * Nothing throws across this boundary. Calls on different streams may run concurrently.
  */
@@ -64,8 +73,10 @@ extern "C" {
  *
  * Integer-valued (more generally: dyadic, exactly representable on the internal 2^-p grid) instances
  * are enumerated exactly and the result is bit-exact. Other real-valued instances are enumerated on a
- * fixed-point grid with a rigorous guard band and re-evaluated in fp64; if the
- * band cannot certify completeness even after widening, ISING_ERR_BAND is returned.
+ * fixed-point grid with a rigorous guard band and re-evaluated in fp64. If more
+ * than 2^20 states lie inside the band of the S-th level (huge levels of states that tie on the grid), a
+ * second enumeration streams exactly those states through the fp64 re-evaluation (ising_stats.passes = 2);
+ * ISING_ERR_BAND is reserved and not returned by the current paths.
  */
 int ising_lowest(const double *J_dev, const double *h_dev, int N, int S,
                  uint64_t *states_out_dev, double *energies_out_dev, void *stream);
@@ -156,7 +167,8 @@ typedef struct ising_stats {
     uint64_t candidates;         /* (E, q) pairs that passed the threshold filter and reached a merge */
     uint32_t kernel_launches;    /* kernels of this library launched */
     uint32_t enum_launches;      /* of which enumeration kernels */
-    uint32_t passes;             /* 1, or more if the guard band had to be widened */
+    uint32_t passes;             /* enumerations of the range: 1; +1 if the single pass overflowed the candidate pool and
+                                    was redone piecewise; +1 for the band pass (more than 2^20 states within the guard band) */
     uint32_t split_retries;      /* launches re-run in halves after a candidate-buffer overflow */
     int32_t  grid_exponent;      /* p: weights were quantised to multiples of 2^-p */
     int32_t  exact;              /* 1 if the grid represents every weight exactly (integer / dyadic instance) */
@@ -165,8 +177,10 @@ typedef struct ising_stats {
     double   total_ms;           /* device time of the whole call */
     int32_t  keep;               /* K: candidates kept per list */
     int32_t  inner_bits;         /* L: unrolled Gray bits per inner block */
-    int32_t  kernel_variant;     /* 1: ising_lowest_alg1. 2: ising_dos. 16: packed 16-bit screen + exact int32 re-forming of hit blocks (default);
-                                    32: int32 add-min per configuration (environment ISING_KERNEL=32) */
+    int32_t  kernel_variant;     /* 1: ising_lowest_alg1. 2: ising_dos. 16: packed 16-bit screen + exact int32 re-forming of hit blocks;
+                                    32: int32 add-min per configuration (environment ISING_KERNEL=32);
+                                    128: as 16 for the ramp-up, the bulk through the tensor-core (tcgen05) screen (default
+                                    for ranges of 2^36 states and more) */
     int32_t  screen_shift;       /* variant 16: one 16-bit unit = 2^screen_shift grid units (0: screen is exact) */
     uint64_t hit_blocks;         /* 1024-configuration blocks that passed the screen and were formed exactly (int32) */
     uint64_t false_hit_blocks;   /* ... of which none held a candidate (the price of the 16-bit screen; 0 for variant 32) */
@@ -198,6 +212,13 @@ int ising_addmin16x2_peak(double ms_target, double *inst_per_s_out_host, void *s
  * measured counterpart of the derived bound of DESIGN.md 5.2 (192 add-mins per clock per SM) and the denominator of
  * bench.py's `roofline.peak`. */
 int ising_addmin_mix_peak(double ms_target, double *addmin_per_s_out_host, void *stream);
+
+/* Self-test of the hardware property the tensor-core screen's proof relies on (csrc/zscreen.cu): one
+ * 128 x 128 x 128 bf16 tcgen05 GEMM of pseudo-random POSITIVE operands spanning 2^-100 .. 2^40, fp32 accumulation in
+ * tensor memory, compared entry by entry with the same sums formed in fp64 from the same bf16 values. Writes the
+ * largest relative UNDER-estimate (ref - D) / ref and over-estimate (D - ref) / ref. The screen's margin (0.02 bits,
+ * i.e. 1.4 %) budgets 2^-14 for this term. */
+int ising_zscreen_selftest(uint32_t seed, double *rel_under_out_host, double *rel_over_out_host, void *stream);
 
 /* Frees the calling thread's cached workspace (device pool, tables, pinned control block). Optional. */
 void ising_release_workspace(void);

@@ -23,7 +23,7 @@ S_MAX = 65536
 EXPORTS = ["ising_lowest", "ising_lowest_range", "ising_lowest_host", "ising_lowest_h0", "ising_lowest_alg1", "ising_dos", "ising_merge_lists", "qubo_lowest",
            "ising_energies", "ising_get_last_stats", "ising_strerror", "ising_last_error", "ising_version",
            "ising_fma_peak", "ising_addmin_peak", "ising_addmin16x2_peak", "ising_addmin_mix_peak",
-           "ising_release_workspace"]
+           "ising_zscreen_selftest", "ising_release_workspace"]
 
 
 class IsingError(RuntimeError):
@@ -100,6 +100,8 @@ def load():
     lib.ising_addmin16x2_peak.argtypes = [ctypes.c_double, ctypes.POINTER(ctypes.c_double), vp]
     lib.ising_addmin_mix_peak.argtypes = [ctypes.c_double, ctypes.POINTER(ctypes.c_double), vp]
     lib.ising_addmin_mix_peak.restype = ctypes.c_int
+    lib.ising_zscreen_selftest.argtypes = [ctypes.c_uint32, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double), vp]
+    lib.ising_zscreen_selftest.restype = ctypes.c_int
     for name in ("ising_lowest", "ising_lowest_range", "ising_lowest_host", "ising_merge_lists", "qubo_lowest",
                  "ising_energies", "ising_get_last_stats", "ising_fma_peak", "ising_addmin_peak", "ising_addmin16x2_peak",
                  "ising_version"):
@@ -352,6 +354,14 @@ def addmin_mix_peak(ms_target: float = 50.0, stream=None) -> float:
     v = ctypes.c_double(0.0)
     _check(load().ising_addmin_mix_peak(float(ms_target), ctypes.byref(v), _stream(stream)), "ising_addmin_mix_peak")
     return v.value
+
+
+def zscreen_selftest(seed: int = 1, stream=None):
+    """(largest relative under-estimate, largest relative over-estimate) of a positive-term tcgen05 bf16 GEMM against
+    fp64 (include/ising.h)."""
+    u, o = ctypes.c_double(0.0), ctypes.c_double(0.0)
+    _check(load().ising_zscreen_selftest(int(seed), ctypes.byref(u), ctypes.byref(o), _stream(stream)), "ising_zscreen_selftest")
+    return u.value, o.value
 
 
 def release_workspace() -> None:

@@ -1002,6 +1002,24 @@ int ising_addmin_mix_peak(double ms_target, double* addmin_per_s_out_host, void*
     return ISING_OK;
 }
 
+int ising_zscreen_selftest(uint32_t seed, double* rel_under_out_host, double* rel_over_out_host, void* stream)
+{
+    t_last_error.clear();
+    if (!rel_under_out_host || !rel_over_out_host) { t_last_error = "null pointer argument"; return ISING_ERR_NULL; }
+    int rc = ensure_workspace();
+    if (rc != ISING_OK) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    double* d = t_ws.out_e;                                  // two doubles of the output staging buffer
+    launch_zselftest(seed, d, st);
+    LAUNCH_CHECK("zselftest_kernel");
+    double h[2] = {0.0, 0.0};
+    CUDA_TRY(cudaMemcpyAsync(h, d, sizeof(h), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    *rel_under_out_host = h[0];
+    *rel_over_out_host = h[1];
+    return ISING_OK;
+}
+
 void ising_release_workspace(void) { if (t_ws.device >= 0) t_ws.release(); }
 
 }  // extern "C"

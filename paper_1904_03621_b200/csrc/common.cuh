@@ -194,6 +194,7 @@ void launch_ztables(const Tables* tab, const Ctrl* ctrl, ZTables* zt, int N, cud
 void launch_zwalk(const Tables* tab, const ZTables* zt, Ctrl* ctrl, Entry* pool, unsigned* hist, const Plan& plan,
                   cudaStream_t st);
 void set_zscreen_attributes();
+void launch_zselftest(unsigned seed, double* out_dev, cudaStream_t st);
 // select.cu
 int  launch_select(Entry* pool, Ctrl* ctrl, unsigned n, int S, const Plan& plan, cudaStream_t st);   // returns kernels launched
 int  launch_compact(const Entry* pool, Entry* pool2, Ctrl* ctrl, const Plan& plan, cudaStream_t st);

@@ -422,6 +422,111 @@ zwalk_kernel(const Tables* __restrict__ tab, const ZTables* __restrict__ zt, Ctr
     }
 }
 
+// ---- self-test of the one hardware property the screen's proof leans on: a tcgen05 bf16 GEMM of POSITIVE terms with
+// fp32 accumulation loses at most a tiny relative amount. One CTA: pseudo-random positive operands spanning many
+// binades (A in 2^[-100, 0], T in 2^[-40, 40], like the kernel's), D from the tensor core against the same sums
+// formed in fp64 on the CUDA cores from the same bf16 values. out[0] = max over entries of (ref - D) / ref
+// (under-estimate), out[1] = max of (D - ref) / ref. ----
+__device__ __forceinline__ unsigned zmix(unsigned x) { x ^= x >> 16; x *= 0x7feb352du; x ^= x >> 15; x *= 0x846ca68bu; x ^= x >> 16; return x; }
+
+__global__ void __launch_bounds__(Z_THREADS) zselftest_kernel(unsigned seed, double* __restrict__ out)
+{
+    extern __shared__ __align__(1024) unsigned char zsmem[];
+    unsigned char* sT = zsmem;
+    unsigned char* sA = zsmem + 32768;
+    __shared__ __align__(8) unsigned long long mbar;
+    __shared__ unsigned s_tmem;
+    __shared__ double s_under, s_over;
+    const int tid = threadIdx.x, warp = tid >> 5;
+    if (tid == 0) { s_under = 0.0; s_over = 0.0; }
+    // row tid of A (thread's own) and row tid of T (n = tid), K = 128 entries each
+    for (int k = 0; k < 128; ++k) {
+        const unsigned ha = zmix(seed ^ (unsigned)(tid * 131 + k) * 2654435761u), ht = zmix(ha + 0x9e3779b9u);
+        const float va = exp2f(-(float)(ha % 100u) - (float)((ha >> 8) & 1023u) / 1024.f);
+        const float vt = exp2f((float)(ht % 81u) - 40.f - (float)((ht >> 8) & 1023u) / 1024.f);
+        const unsigned off = (unsigned)(tid >> 3) * Z_SBO + (unsigned)(k >> 3) * Z_LBO + (unsigned)(tid & 7) * 16u + (unsigned)(k & 7) * 2u;
+        *reinterpret_cast<__nv_bfloat16*>(sA + off) = __float2bfloat16_rn(va);
+        *reinterpret_cast<__nv_bfloat16*>(sT + off) = __float2bfloat16_rn(vt);
+    }
+    if (tid == 0) {
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"(smem_u32(&mbar)), "r"(1));
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 0) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" :: "r"(smem_u32(&s_tmem)), "r"(128));
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+    }
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    const unsigned tmem = s_tmem;
+    if (tid == 0) {
+        const unsigned a0 = smem_u32(sA), b0 = smem_u32(sT);
+#pragma unroll
+        for (int ks = 0; ks < 8; ++ks) {
+            const unsigned long long da = umma_desc(a0 + (unsigned)ks * 2u * Z_LBO);
+            const unsigned long long db = umma_desc(b0 + (unsigned)ks * 2u * Z_LBO);
+            const unsigned acc = ks > 0 ? 1u : 0u;
+            asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+                         "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
+                         :: "r"(tmem), "l"(da), "l"(db), "r"(Z_IDESC), "r"(acc) : "memory");
+        }
+        asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(smem_u32(&mbar)) : "memory");
+    }
+    asm volatile("{\n\t.reg .pred P1;\n\tSWAIT_%=:\n\t"
+                 "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n\t"
+                 "@P1 bra SDONE_%=;\n\tbra SWAIT_%=;\n\tSDONE_%=:\n\t}" :: "r"(smem_u32(&mbar)), "r"(0) : "memory");
+    __syncwarp();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    double under = 0.0, over = 0.0;
+    for (int c = 0; c < 4; ++c) {
+        unsigned v[32];
+        const unsigned taddr = tmem + ((unsigned)(warp * 32) << 16) + (unsigned)(c * 32);
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+                     "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+                     "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+                     : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+                       "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]),
+                       "=r"(v[16]), "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]),
+                       "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+                     : "r"(taddr) : "memory");
+        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+        for (int j = 0; j < 32; ++j) {
+            const int n = c * 32 + j;
+            double ref = 0.0;
+            for (int k = 0; k < 128; ++k) {
+                const unsigned oa = (unsigned)(tid >> 3) * Z_SBO + (unsigned)(k >> 3) * Z_LBO + (unsigned)(tid & 7) * 16u + (unsigned)(k & 7) * 2u;
+                const unsigned ot = (unsigned)(n >> 3) * Z_SBO + (unsigned)(k >> 3) * Z_LBO + (unsigned)(n & 7) * 16u + (unsigned)(k & 7) * 2u;
+                ref += (double)__bfloat162float(*reinterpret_cast<const __nv_bfloat16*>(sA + oa)) *
+                       (double)__bfloat162float(*reinterpret_cast<const __nv_bfloat16*>(sT + ot));
+            }
+            const double d = (double)__uint_as_float(v[j]);
+            if (ref > 0.0) {
+                under = fmax(under, (ref - d) / ref);
+                over = fmax(over, (d - ref) / ref);
+            }
+        }
+    }
+    // positive doubles order like their bit patterns
+    atomicMax(reinterpret_cast<unsigned long long*>(&s_under), (unsigned long long)__double_as_longlong(under));
+    atomicMax(reinterpret_cast<unsigned long long*>(&s_over), (unsigned long long)__double_as_longlong(over));
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    if (tid == 0) { out[0] = s_under; out[1] = s_over; }
+    __syncwarp();
+    if (warp == 0) {
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(tmem), "r"(128));
+    }
+}
+
+void launch_zselftest(unsigned seed, double* out_dev, cudaStream_t st)
+{
+    cudaFuncSetAttribute(zselftest_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, Z_SMEM_BYTES);
+    zselftest_kernel<<<1, Z_THREADS, Z_SMEM_BYTES, st>>>(seed, out_dev);
+}
+
 void launch_ztables(const Tables* tab, const Ctrl* ctrl, ZTables* zt, int N, cudaStream_t st)
 {
     ztables_kernel<<<1, 1024, 0, st>>>(tab, ctrl, zt, N);

@@ -881,3 +881,62 @@ def test_first_calls_from_two_threads(B, tmp_path):
     J, h = I.complete_gaussian(20, seed=7)
     qo, _ = oracle.lowest(J, h, 6000)
     assert np.load(out).tolist() == qo.tolist()
+
+
+# ---------- the tensor-core (tcgen05) screen of zscreen.cu, forced on at sizes the oracle reaches ----------
+@pytest.mark.parametrize("name", ["gauss24", "gauss26", "gauss27_h2", "int26", "sparse25", "mattis30", "wide24", "fields27",
+                                  "zero24"])
+def test_tensor_core_screen_small(B, name):
+    """ISING_Z_MIN_LOG2 = 24 sends everything after the first eighth of the range through the partition-function
+    screen (probe + bulk, or the packed kernel if the probe flags too much): the list must be the oracle's whatever
+    the screen does, on Gaussian, integer (heavy ties), sparse, closed-form, wide-range and degenerate instances."""
+    S = 100
+    if name == "gauss24":
+        J, h = I.complete_gaussian(24, seed=2401)
+    elif name == "gauss26":
+        J, h = I.complete_gaussian(26, seed=2601); S = 1000
+    elif name == "gauss27_h2":
+        J, h = I.complete_gaussian(27, seed=2701, h_scale=2.0); S = 16
+    elif name == "int26":
+        J, h = I.random_integer(26, seed=2626, wmax=3, density=0.5); S = 500
+    elif name == "sparse25":
+        J, h = I.random_integer(25, seed=2525, wmax=1, density=0.12); S = 300
+    elif name == "mattis30":
+        J, h, _ = I.mattis(30, seed=3030); S = 62
+    elif name == "wide24":
+        J, h = _wide_range_instance(24, 2424); S = 200
+    elif name == "fields27":
+        J, h = I.fields_only(27, seed=27); S = 50
+    else:
+        J, h = np.zeros((24, 24)), np.zeros(24); S = 40
+    q, e = _with_env({"ISING_Z_MIN_LOG2": 24}, lambda: gpu_lowest(B, J, h, S))
+    st = B.last_stats()
+    assert st.configs == 1 << len(h) and st.kernel_variant in (16, 128)
+    if name == "mattis30":
+        qo, eo = oracle.lowest_gray(J, h, S)
+    else:
+        qo, eo = oracle.lowest(J, h, S)
+    assert_exact(q, e, qo, eo)
+
+
+def test_tensor_core_screen_is_used_and_agrees_with_the_other_kernels(B, golden_dir):
+    """cfg3 (2^36 states): by default the bulk goes through the tensor-core screen (kernel_variant 128); the packed
+    kernel alone and the int32 kernel alone must return the same list, which is the stored oracle list."""
+    c = I.baseline_config(3)
+    qo, eo = load_golden(os.path.join(golden_dir, "cfg3.txt"))
+    q, e = gpu_lowest(B, c.J, c.h, c.S)
+    assert B.last_stats().kernel_variant == 128
+    assert_exact(q, e, qo[:c.S], eo[:c.S])
+    for v in (16, 32):
+        q2, e2 = _with_kernel(v, lambda: gpu_lowest(B, c.J, c.h, c.S))
+        assert B.last_stats().kernel_variant == v
+        assert_exact(q2, e2, qo[:c.S], eo[:c.S])
+
+
+def test_tensor_core_accumulation_selftest(B):
+    """The hardware property the screen's proof budgets 2^-14 for: a bf16 tcgen05 GEMM of positive terms
+    spanning 140 binades, fp32 accumulation, against fp64 sums of the same bf16 values."""
+    for seed in (1, 2, 3, 12345):
+        under, over = B.zscreen_selftest(seed)
+        assert 0.0 <= under < 2.0 ** -14, under
+        assert 0.0 <= over < 2.0 ** -14, over
