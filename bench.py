@@ -8,8 +8,12 @@ selected, the survivors re-evaluated in fp64 and the S lowest written (SURVEY.md
 
   value          configurations evaluated per second, whole job, inputs resident in HBM, CUDA-event timed
   e2e            same through the host-buffer API: pinned HOST buffers in and out, copies inside the timed region
-  roofline       the enumeration kernel (packed 16-bit screen) against the MEASURED rate of its instruction mix
-  roofline_int32 the int32 kernel (arithmetic no narrower than the paper's) on the same full space, same invocation
+  roofline       the dominant kernel: the tensor-core screen (zwalk_kernel, one 128x128x128 bf16 tcgen05 GEMM per 2^21
+                 configurations, 2 flop per configuration) against the measured cuBLAS bf16 rate of MEASURED_PEAKS.json
+  roofline_packed16 / roofline_int32
+                 the same full space, same invocation, through the packed 16-bit ALU screen only (ISING_KERNEL=16) and
+                 through the int32 kernel (ISING_KERNEL=32: arithmetic no narrower than the paper's), each against the
+                 MEASURED rate of its own instruction mix
   cpu_baseline   the CPU oracle, as it stands, on a bounded prefix of the same instance (rank 0, N=1 only)
 
 N > 1 (torchrun): the path shards by ranges of q: ONE instance, one aligned state range per rank,
@@ -64,7 +68,8 @@ def parse_args():
     ap.add_argument("--n-spins", type=int, default=0,
                     help="replace the config's instance by a complete Gaussian instance of this many spins (S as in the "
                          "config); for multi-GPU runs, e.g. 50 or 52")
-    ap.add_argument("--no-int32", action="store_true", help="skip the int32-kernel pass (one more full enumeration)")
+    ap.add_argument("--no-int32", action="store_true",
+                    help="skip the ALU-kernel passes (one more full enumeration each: packed 16-bit 8 s, int32 18 s at N=48)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -274,6 +279,8 @@ def main():
     launches = 0
     enum_configs = 0
     hit_blocks = false_hit_blocks = 0
+    z_ms = 0.0
+    z_configs = z_blocks = z_flagged = z_launches = 0
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     for _ in range(args.steps):
         flush.zero_()                       # L2 flush between timed iterations (outside the event bracket)
@@ -288,6 +295,8 @@ def main():
         launches += st.kernel_launches
         hit_blocks += st.hit_blocks
         false_hit_blocks += st.false_hit_blocks
+        z_ms += st.z_ms; z_configs += st.z_configs; z_blocks += st.z_blocks
+        z_flagged += st.z_flagged_blocks; z_launches += st.z_launches
     barrier()
     t_wall1 = time.perf_counter()
     clocks = sampler.summary(t_wall0, t_wall1)
@@ -317,26 +326,30 @@ def main():
         assert qh.numpy().view(np.uint64).tolist() == result_states
         e2e = {"seconds": e2e_s, "h2d": (N * N + N) * 8, "d2h": S * 16}
 
-    # ---- the int32 kernel (32-bit exact add-min per configuration: no narrower than the paper's arithmetic) on the
-    # same workload, timed with its own CUDA events; fewer steps (it is 2.2x slower), rank-local like `roofline` ----
-    int32 = None
+    # ---- the ALU kernels on the same workload, each timed with its own CUDA events; fewer steps (they are 14x and
+    # 32x slower than the default path), rank-local like `roofline`: ISING_KERNEL=16 = packed 16-bit screen only (the
+    # round-1 default), ISING_KERNEL=32 = 32-bit exact add-min per configuration (no narrower than the paper's) ----
+    alu_runs = {}
     if not args.no_int32 and not sharded_mode:
-        os.environ["ISING_KERNEL"] = "32"
-        try:
-            n32 = max(1, min(args.steps, 2))
-            ms32 = e32 = 0.0
-            c32 = 0
-            for _ in range(n32):
-                ev0.record(stream)
-                q32, _ = B.ising_lowest_range(J, h, S, 0, q_end, stream=stream)
-                ev1.record(stream); ev1.synchronize()
-                st32 = B.last_stats()
-                assert st32.kernel_variant == 32
-                ms32 += ev0.elapsed_time(ev1); e32 += st32.enum_ms; c32 += st32.configs
-            assert B.states_to_numpy(q32).tolist() == result_states       # same list as the packed kernel
-            int32 = {"ms_per_step": ms32 / n32, "enum_ms": e32, "configs": c32, "steps": n32}
-        finally:
-            os.environ.pop("ISING_KERNEL", None)
+        for kv, nsteps in ((16, 1 if st.kernel_variant == 128 else 0), (32, max(1, min(args.steps, 2)))):
+            if nsteps == 0:
+                continue
+            os.environ["ISING_KERNEL"] = str(kv)
+            try:
+                msk = ek = 0.0
+                ck = 0
+                for _ in range(nsteps):
+                    ev0.record(stream)
+                    qk, _ = B.ising_lowest_range(J, h, S, 0, q_end, stream=stream)
+                    ev1.record(stream); ev1.synchronize()
+                    stk = B.last_stats()
+                    assert stk.kernel_variant == kv
+                    msk += ev0.elapsed_time(ev1); ek += stk.enum_ms; ck += stk.configs
+                assert B.states_to_numpy(qk).tolist() == result_states       # same list as the default path
+                alu_runs[kv] = {"ms_per_step": msk / nsteps, "enum_ms": ek, "configs": ck, "steps": nsteps,
+                                "enum_launches": stk.enum_launches}
+            finally:
+                os.environ.pop("ISING_KERNEL", None)
     sampler.stop()
 
     # max over ranks of the device time
@@ -349,38 +362,86 @@ def main():
 
     if rank == 0:
         sm_max_hz = 1.965e9
+        peaks = None
         try:
             peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
             sm_max_hz = float(peaks.get("sm_max_mhz", 1965.0)) * 1e6
         except Exception:
-            pass
+            peaks = None
         sms = torch.cuda.get_device_properties(local_rank).multi_processor_count
-        per_inst = 2 if st.kernel_variant == 16 else 1                 # add-mins (configurations) per lane instruction
-        fused_nominal = sms * ALU_LANES_PER_CLK_PER_SM * sm_max_hz * per_inst     # add-min ops / s, fused form only
-        fused_live = addmin16x2_peak * 2 if st.kernel_variant == 16 else addmin_peak
-        derived_mix = sms * MIX_BOUND_CONFIGS_PER_CLK_PER_SM * sm_max_hz
-        # the peak the fraction is quoted against is MEASURED in this run: for the packed kernel the best of the two
-        # register-only microbenchmarks of its own instruction forms (fused VIADDMNMX.U16x2 alone; fused + split mix)
-        peak_live = max(fused_live, addmin_mix_peak) if st.kernel_variant == 16 else fused_live
-        kname = "ising::walk_kernel<Inner16>" if st.kernel_variant == 16 else "ising::walk_kernel<Inner32>"
         fma_nominal = sms * FMA_LANES_PER_CLK_PER_SM * sm_max_hz       # FMA / s
-        achieved = float(enum_configs) / (enum_ms * 1e-3)   # this rank's kernel: one add-min per configuration
-        traffic, traffic_source = None, None
-        tpath = os.path.join(ROOT, "profiles", "enumerate_dram_bytes_per_launch.txt")
-        if os.path.exists(tpath):
+        derived_mix = sms * MIX_BOUND_CONFIGS_PER_CLK_PER_SM * sm_max_hz
+
+        def profile_number(fname):
+            """First number of a one-line file under profiles/ (an ncu capture of one launch; its source says so)."""
             try:
-                txt = open(tpath).read().split()
-                traffic = float(txt[0])
-                traffic_source = ("ncu --set full capture of one launch of this kernel (dram__bytes_read.sum + "
-                                  "dram__bytes_write.sum), stored in profiles/enumerate_dram_bytes_per_launch.txt; "
-                                  "not re-measured in this run")
+                return float(open(os.path.join(ROOT, "profiles", fname)).read().split()[0])
             except Exception:
-                traffic = None
+                return None
+
+        def alu_roofline(variant, achieved, launches, ms):
+            """Roofline object of an ALU enumeration kernel: one add-min per configuration against the MEASURED rate of
+            its own instruction forms (register-only microbenchmarks run above, in this invocation)."""
+            packed = variant == 16
+            fused_live = addmin16x2_peak * 2 if packed else addmin_peak
+            peak = max(fused_live, addmin_mix_peak) if packed else fused_live
+            fused_nominal = sms * ALU_LANES_PER_CLK_PER_SM * sm_max_hz * (2 if packed else 1)
+            r = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "add-min/s", "frac": achieved / peak,
+                 "kernel": "ising::walk_kernel<Inner16>" if packed else "ising::walk_kernel<Inner32>",
+                 "launches": launches, "avg_launch_ms": ms / max(launches, 1),
+                 "peak_source": ("MEASURED in this run: max of ising_addmin16x2_peak x 2 (fused VIADDMNMX.U16x2 only) and "
+                                 "ising_addmin_mix_peak (fused + IMAD/IMAD/VIMNMX3.U16x2 mix), register-only loops on the "
+                                 "whole GPU" if packed else
+                                 "MEASURED in this run: ising_addmin_peak (VIADDMNMX.S32, register-only loop)"),
+                 "fused_only_nominal": fused_nominal, "frac_of_fused_only_nominal": achieved / fused_nominal}
+            if packed:
+                r.update({"fused_only_measured": fused_live, "mix_measured": addmin_mix_peak,
+                          "mix_bound_derived": derived_mix, "frac_of_mix_bound_derived": achieved / derived_mix,
+                          "mix_bound_note": "derived LP bound (ALU pipe 16 lanes/clk, 1 issue slot/clk per sub-partition); "
+                                            "the measured mix does not reach it (DESIGN.md 5.2)"})
+            return r
+
+        enum_rate = float(enum_configs) / (enum_ms * 1e-3)     # all enumeration launches of this rank
+        if st.kernel_variant == 128:
+            # dominant kernel: the tensor-core screen. Algorithmic work = the GEMM: one 128 x 128 x 128 bf16 product per
+            # 2^21 configurations = 2 flop per configuration (DESIGN.md 5.1c); time = CUDA events around its launches.
+            bf16_burst = float(peaks.get("bf16_tflops", 1590.0)) if peaks else 1590.0
+            bf16_sust = float(peaks.get("bf16_tflops_sustained", 1400.0)) if peaks else 1400.0
+            z_rate = float(z_configs) / (z_ms * 1e-3)
+            achieved_tf = 2.0 * z_rate * 1e-12
+            traffic = profile_number("zwalk_dram_bytes_per_launch.txt")
+            roofline = {"bound": "tensor", "achieved": achieved_tf, "peak": bf16_sust, "unit": "TFLOP/s",
+                        "frac": achieved_tf / bf16_sust, "traffic": traffic,
+                        "traffic_source": ("ncu --set full capture of one launch of this kernel (dram__bytes_read.sum + "
+                                           "dram__bytes_write.sum), stored in profiles/zwalk_dram_bytes_per_launch.txt; "
+                                           "not re-measured in this run; algorithmic HBM bytes per configuration: 0")
+                                          if traffic is not None else None,
+                        "kernel": "ising::zwalk_kernel", "launches": z_launches,
+                        "avg_launch_ms": z_ms / max(z_launches, 1),
+                        "flop_per_configuration": 2.0, "configs_per_s_in_kernel": z_rate,
+                        "share_of_enumeration_time": z_ms / enum_ms, "share_of_configurations": z_configs / enum_configs,
+                        "peak_source": ("MEASURED_PEAKS.json bf16_tflops_sustained (cuBLAS bf16 GEMM back to back; the kernel "
+                                        "is timed inside a long step)" if peaks else "fallback of B200_PROFILING.md"),
+                        "peak_burst": bf16_burst, "frac_of_burst": achieved_tf / bf16_burst,
+                        "peak_nominal": 2250.0, "frac_of_nominal": achieved_tf / 2250.0,
+                        "blocks_screened": z_blocks, "blocks_flagged": z_flagged,
+                        "note": "the GEMM is the algorithmic work of the screen; around it every thread generates its "
+                                "operand row and folds its accumulator row on the CUDA cores (DESIGN.md 5.1c), and the "
+                                "first 2^35 states go through the packed ALU kernel (roofline_packed16)"}
+            dtype = "bf16 tensor-core screen (fp32 accumulate) + int16x2 screen + int32 exact (fp64 output)"
+        else:
+            roofline = alu_roofline(st.kernel_variant, enum_rate, enum_launches, enum_ms)
+            traffic = profile_number("enumerate_dram_bytes_per_launch.txt")
+            roofline["traffic"] = traffic
+            roofline["traffic_source"] = ("ncu --set full capture of one launch of this kernel, stored in "
+                                          "profiles/enumerate_dram_bytes_per_launch.txt; not re-measured in this run"
+                                          if traffic is not None else None)
+            dtype = "int16x2 screen + int32 exact (fp64 output)" if st.kernel_variant == 16 else "int32 (fp64 output)"
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": dev_ms_max / args.steps, "higher_is_better": True,
             "scaling": "strong" if (sharded_mode and world > 1) else "weak", "vs_baseline": None,
-            "dtype": "int16x2 screen + int32 exact (fp64 output)" if st.kernel_variant == 16 else "int32 (fp64 output)",
+            "dtype": dtype,
             "data": "synthetic",
             "config": {"workload": f"BASELINE.json configs[{args.config - 1}]: {inst.name}, N={N}, S={S}, "
                                    f"states [0, 2^{q_end.bit_length() - 1}) of 2^{N} per step",
@@ -398,33 +459,23 @@ def main():
                                   "frac_of_measured": value / world * N / fma_peak,
                                   "frac_of_nominal": value / world * N / fma_nominal,
                                   "fma_per_s_measured": fma_peak, "fma_per_s_nominal": fma_nominal},
-            "roofline": {"bound": "alu", "achieved": achieved, "peak": peak_live, "unit": "add-min/s",
-                         "frac": achieved / peak_live, "traffic": traffic, "traffic_source": traffic_source,
-                         "kernel": kname, "launches": enum_launches,
-                         "avg_launch_ms": enum_ms / max(enum_launches, 1),
-                         "peak_source": ("MEASURED in this run: max of ising_addmin16x2_peak x 2 (fused VIADDMNMX.U16x2 "
-                                         "only) and ising_addmin_mix_peak (fused + IMAD/IMAD/VIMNMX3.U16x2 mix), "
-                                         "register-only loops on the whole GPU" if st.kernel_variant == 16 else
-                                         "MEASURED in this run: ising_addmin_peak (VIADDMNMX.S32, register-only loop)"),
-                         "fused_only_measured": fused_live, "mix_measured": addmin_mix_peak,
-                         "fused_only_nominal": fused_nominal, "frac_of_fused_only_nominal": achieved / fused_nominal,
-                         "mix_bound_derived": derived_mix, "frac_of_mix_bound_derived": achieved / derived_mix,
-                         "mix_bound_note": "derived LP bound (ALU pipe 16 lanes/clk, 1 issue slot/clk per sub-partition); "
-                                           "the measured mix does not reach it: VIMNMX3.U16x2 and IMAD do not overlap "
-                                           "with VIADDMNMX as the LP assumes (DESIGN.md 5.2)",
-                         "viaddmnmx_s32_per_s_live": addmin_peak, "viaddmnmx_u16x2_per_s_live": addmin16x2_peak},
+            "roofline": roofline,
+            "enumeration_all_launches": {"configs_per_s": enum_rate, "launches": enum_launches, "ms": enum_ms},
+            "microbenchmarks_live": {"ffma_per_s": fma_peak, "viaddmnmx_s32_per_s": addmin_peak,
+                                     "viaddmnmx_u16x2_inst_per_s": addmin16x2_peak, "addmin_mix_per_s": addmin_mix_peak},
             "gpu_launches": launches,
             "clocks": clocks,
         }
-        if int32:
-            a32 = float(int32["configs"]) / (int32["enum_ms"] * 1e-3)
-            line["roofline_int32"] = {"bound": "alu", "kernel": "ising::walk_kernel<Inner32>", "achieved": a32,
-                                      "peak": addmin_peak, "unit": "add-min/s", "frac": a32 / addmin_peak,
-                                      "peak_source": "MEASURED in this run: ising_addmin_peak (VIADDMNMX.S32)",
-                                      "time_to_S_lowest_s": int32["ms_per_step"] * 1e-3,
-                                      "configs_per_s": float(configs_per_step) / (int32["ms_per_step"] * 1e-3),
-                                      "steps": int32["steps"], "same_list_as_packed_kernel": True,
-                                      "dtype": "int32 (fp64 output)"}
+        for kv, key in ((16, "roofline_packed16"), (32, "roofline_int32")):
+            if kv in alu_runs:
+                rr = alu_runs[kv]
+                ak = float(rr["configs"]) / (rr["enum_ms"] * 1e-3)
+                obj = alu_roofline(kv, ak, rr["enum_launches"] * rr["steps"], rr["enum_ms"])
+                obj.update({"time_to_S_lowest_s": rr["ms_per_step"] * 1e-3,
+                            "configs_per_s": float(configs_per_step) / (rr["ms_per_step"] * 1e-3),
+                            "steps": rr["steps"], "same_list_as_default_path": True,
+                            "dtype": "int16x2 screen + int32 exact (fp64 output)" if kv == 16 else "int32 (fp64 output)"})
+                line[key] = obj
         if e2e:
             line["e2e"] = {"value": total_configs / e2e_s_max, "unit": UNIT,
                            "h2d_bytes_per_step": e2e["h2d"], "d2h_bytes_per_step": e2e["d2h"]}

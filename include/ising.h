@@ -184,6 +184,13 @@ typedef struct ising_stats {
     int32_t  screen_shift;       /* variant 16: one 16-bit unit = 2^screen_shift grid units (0: screen is exact) */
     uint64_t hit_blocks;         /* 1024-configuration blocks that passed the screen and were formed exactly (int32) */
     uint64_t false_hit_blocks;   /* ... of which none held a candidate (the price of the 16-bit screen; 0 for variant 32) */
+    /* tensor-core screen (variant 128 only, else 0) */
+    double   z_ms;               /* device time of the launches of the tensor-core screen kernel (part of enum_ms) */
+    uint64_t z_configs;          /* configurations those launches covered (probe + bulk) */
+    uint64_t z_blocks;           /* 2^14-configuration blocks screened by one row of a 128 x 128 x 128 GEMM each */
+    uint64_t z_flagged_blocks;   /* ... of which flagged and formed exactly (16 blocks of 1024 each, counted in hit_blocks) */
+    uint32_t z_launches;         /* launches of the tensor-core screen kernel (part of enum_launches) */
+    uint32_t reserved0;
 } ising_stats;
 
 int ising_get_last_stats(ising_stats *out_host);

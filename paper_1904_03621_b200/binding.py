@@ -40,7 +40,9 @@ class _Stats(ctypes.Structure):
                 ("epsilon", ctypes.c_double), ("enum_ms", ctypes.c_double), ("total_ms", ctypes.c_double),
                 ("keep", ctypes.c_int32), ("inner_bits", ctypes.c_int32),
                 ("kernel_variant", ctypes.c_int32), ("screen_shift", ctypes.c_int32),
-                ("hit_blocks", ctypes.c_uint64), ("false_hit_blocks", ctypes.c_uint64)]
+                ("hit_blocks", ctypes.c_uint64), ("false_hit_blocks", ctypes.c_uint64),
+                ("z_ms", ctypes.c_double), ("z_configs", ctypes.c_uint64), ("z_blocks", ctypes.c_uint64),
+                ("z_flagged_blocks", ctypes.c_uint64), ("z_launches", ctypes.c_uint32), ("reserved0", ctypes.c_uint32)]
 
 
 @dataclass
@@ -62,6 +64,11 @@ class Stats:
     screen_shift: int
     hit_blocks: int = 0
     false_hit_blocks: int = 0
+    z_ms: float = 0.0
+    z_configs: int = 0
+    z_blocks: int = 0
+    z_flagged_blocks: int = 0
+    z_launches: int = 0
 
 
 _lib = None
@@ -153,7 +160,7 @@ def last_stats() -> Stats:
     _check(load().ising_get_last_stats(ctypes.byref(s)), "ising_get_last_stats")
     return Stats(s.configs, s.candidates, s.kernel_launches, s.enum_launches, s.passes, s.split_retries,
                  s.grid_exponent, bool(s.exact), s.epsilon, s.enum_ms, s.total_ms, s.keep, s.inner_bits, s.kernel_variant, s.screen_shift,
-                 s.hit_blocks, s.false_hit_blocks)
+                 s.hit_blocks, s.false_hit_blocks, s.z_ms, s.z_configs, s.z_blocks, s.z_flagged_blocks, s.z_launches)
 
 
 def ising_lowest_range(J, h, S: int, q_begin: int, q_end: int, stream=None, out=None):

@@ -165,6 +165,8 @@ struct Run {
     unsigned long long q_begin, q_end;
     cudaStream_t st;
     double enum_ms;
+    double z_ms;                    // of which in launches of the tensor-core screen
+    unsigned long long z_configs;   // configurations those launches covered
     bool done;                      // the single pass wrote the outputs and recorded the end event
 };
 
@@ -312,10 +314,14 @@ int run_single_pass(Run& r, unsigned long long* states_out, double* energies_out
         CUDA_TRY(cudaEventRecord(ws.ev[3], r.st));
         return ISING_OK;
     };
+    bool last_was_z = false;
+    unsigned long long last_z_configs = 0;
     auto add_elapsed = [&]() -> int {
         float ms = 0.f;
         CUDA_TRY(cudaEventElapsedTime(&ms, ws.ev[2], ws.ev[3]));
         r.enum_ms += ms;
+        if (last_was_z) { r.z_ms += ms; r.z_configs += last_z_configs; }
+        last_was_z = false;
         return ISING_OK;
     };
     if (direct) {
@@ -375,6 +381,9 @@ int run_single_pass(Run& r, unsigned long long* states_out, double* energies_out
             if (rc != ISING_OK) return rc;
             r.stats->kernel_launches += 3;
             r.stats->enum_launches += 1;
+            r.stats->z_launches += 1;
+            last_was_z = true;
+            last_z_configs = p0;
             rc = read_ctrl(r);
             if (rc != ISING_OK) return rc;
             if ((rc = add_elapsed()) != ISING_OK) return rc;
@@ -400,9 +409,11 @@ int run_single_pass(Run& r, unsigned long long* states_out, double* energies_out
                 LAUNCH_CHECK("zwalk_kernel");
                 r.stats->kernel_launches += 1;
                 r.stats->enum_launches += 1;
+                r.stats->z_launches += 1;
                 return ISING_OK;
             });
             if (rc != ISING_OK) return rc;
+            if (z_ok) { last_was_z = true; last_z_configs = r.q_end - (r.q_begin + 2 * p0); }
         } else if (cur != r.q_end) {
             t_last_error = "internal: work plan does not cover the range";
             return ISING_ERR_INTERNAL;
@@ -422,6 +433,8 @@ int run_single_pass(Run& r, unsigned long long* states_out, double* energies_out
     r.stats->configs += range;
     if (c.pool_overflow) { *redo = true; return ISING_OK; }
     r.stats->candidates += c.count;
+    r.stats->z_blocks = c.z_steps;
+    r.stats->z_flagged_blocks = c.z_flagged;
     if (c.final_state == 1) { r.stats->keep = (int)c.kept; r.done = true; return ISING_OK; }
     if (c.final_state != 2 || c.count2 < (unsigned)r.S) {
         t_last_error = "internal: fewer candidates than requested states";
@@ -576,7 +589,7 @@ int run_lowest(const double* J, const double* h, const double* Jorig, const doub
     r.keep_cap = 1u << env_int("ISING_KEEP_CAP_LOG2", 20, 5, 20);
     while (r.keep_cap < (unsigned)S) r.keep_cap <<= 1;
     const int path = env_int("ISING_PATH", 0, 0, 1);        // 1: skip the single pass (tests of the host-sequenced path)
-    r.q_begin = q_begin; r.q_end = q_end; r.st = st; r.enum_ms = 0.0; r.done = false;
+    r.q_begin = q_begin; r.q_end = q_end; r.st = st; r.enum_ms = 0.0; r.z_ms = 0.0; r.z_configs = 0; r.done = false;
     const int rb = floor_log2(q_end - q_begin - 1) + 1;     // bits of the range
     r.qshift = rb > 31 ? rb - 31 : 0;                       // (range >> qshift) < 2^32 - 1
 
@@ -609,7 +622,10 @@ int run_lowest(const double* J, const double* h, const double* Jorig, const doub
 
     if (redo) {
         // the single pass was void (or skipped): the same range again, host-sequenced
-        if (path == 0) { stats.passes += 1; stats.configs = 0; stats.candidates = 0; }
+        if (path == 0) {
+            stats.passes += 1; stats.configs = 0; stats.candidates = 0;
+            stats.z_blocks = stats.z_flagged_blocks = 0; stats.z_launches = 0; r.z_ms = 0.0; r.z_configs = 0;
+        }
         restart_kernel<<<1, 1, 0, st>>>(ws.ctrl, tau_pack(TAU_INF, QC_NONE));
         LAUNCH_CHECK("restart_kernel");
         stats.kernel_launches += 1;
@@ -668,6 +684,8 @@ int run_lowest(const double* J, const double* h, const double* Jorig, const doub
     CUDA_TRY(cudaEventElapsedTime(&total_ms, ws.ev[0], ws.ev[1]));
     stats.enum_ms = r.enum_ms;
     stats.total_ms = total_ms;
+    stats.z_ms = r.z_ms;
+    stats.z_configs = r.z_configs;
     stats.hit_blocks = ws.h_ctrl->hits;
     stats.false_hit_blocks = ws.h_ctrl->false_hits;
     t_stats = stats;
