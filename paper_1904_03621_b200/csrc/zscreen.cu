@@ -25,8 +25,9 @@
 // Why the screen is rigorous (DESIGN.md section 6b has the full argument):
 //   * all terms are positive, so rounding only perturbs Z relatively: T and a are rounded to bf16 (2^-9 each, to
 //     nearest), the fp32 products inside the tensor core are exact, accumulation, the u-fold and the factor chain add
-//     < 2^-11; in the log domain that is < 0.007 bits, and L itself is good to 1e-3 bits. The test flags a block
-//     unless  log2(Z~) + L < -0.02 ;
+//     < 2^-11; in the log domain that is < 0.007 bits, and L -- one fp32 multiply-add of an EXACT integer,
+//     L = lambda (tauE - Eh + 2 sum_i max(Phi_i, 0)) - t0 -- is good to 2^-22 |L| < 1e-4 bits wherever the test can
+//     go either way (|L| < 200). The test flags a block unless  log2(Z~) + L < -0.02 ;
 //   * underflow: a term of a configuration with E <= tauE has  log2 a + log2 T + log2 u >= -L; with |log2 T| <= THETA
 //     (lambda is chosen from the range of C') none of its partial products is below 2^-(L + THETA), so for
 //     L <= L_SAFE = 126 - THETA - 8 it cannot underflow; blocks with L > L_SAFE are flagged unconditionally
@@ -240,19 +241,19 @@ zwalk_kernel(const Tables* __restrict__ tab, const ZTables* __restrict__ zt, Ctr
         //   bit set multiplies the weight by 2^y, y = 2 lambda Phi; normalised so that the larger of the two factors of
         //   a spin is exactly 1. a[lo] = product over the 7 lo spins, 128 values, bf16, canonical layout; products in
         //   packed fp32 pairs (FMUL2): pair p of Q holds lo = 2p (low lane: spin 0 down) and 2p + 1 (spin 0 up).
-        // Returns the mid-spin factors (for the fold) and  sum_i max(y_i, 0) - t0  (the instance part of L).
-        auto gen_row = [&](int buf, const int (&Ph)[ZB], float (&m0)[7], float (&m1)[7], float& lpb) {
+        // Returns the mid-spin factors (for the fold). The log-domain offset L is formed from EXACT integers,
+        // L = lambda (tauE - Eh + 2 sum_i max(Phi_i, 0)) - t0 (spos below), so that its error is RELATIVE (2^-23 |L|)
+        // however large the fields are in grid units (summing the fp32 terms lambda (tauE - Eh) and 2 lambda Phi_i
+        // separately would cancel catastrophically on instances with strong fields and weak couplings in the block).
+        auto gen_row = [&](int buf, const int (&Ph)[ZB], float (&m0)[7], float (&m1)[7]) {
             float r0[ZB], r1[ZB];
-            float acc = -t0;
 #pragma unroll
             for (int i = 0; i < ZB; ++i) {
                 const float y = two_lambda * (float)Ph[i];
                 const float e = ex2f(-fabsf(y));
                 r1[i] = y >= 0.f ? 1.f : e;
                 r0[i] = y >= 0.f ? e : 1.f;
-                acc += fmaxf(y, 0.f);
             }
-            lpb = acc;
 #pragma unroll
             for (int i = 0; i < 7; ++i) { m0[i] = r0[7 + i]; m1[i] = r1[7 + i]; }
             unsigned long long Q[16];
@@ -311,9 +312,14 @@ zwalk_kernel(const Tables* __restrict__ tab, const ZTables* __restrict__ zt, Ctr
         //      two accumulators -- was measured and dropped: the larger footprint leaves two CTAs per SM, and with eight
         //      warps per SM the dependent chains of the row generation and the fold are not hidden: 4.2e14 against
         //      4.9e14 configurations/s.) ----
-        float m0[7], m1[7], lpb;
+        float m0[7], m1[7];
         for (unsigned t = 0; t < nsteps; ++t) {
-            gen_row(0, Phi, m0, m1, lpb);
+            int spos = 0;                                   // sum_i max(Phi_i, 0) of THIS step's fields
+#pragma unroll
+            for (int i = 0; i < ZB; ++i) spos += max(Phi[i], 0);
+            // (a threshold read a moment ago is never tighter than the current one: conservative)
+            const float Lp = fmaf(lambda, (float)(tauE - Eh + 2 * spos), -t0);      // |integer| < 2^31 (4 Wq + 2^30)
+            gen_row(0, Phi, m0, m1);
             asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
             __syncthreads();       // every A row is written; every TMEM read of the previous step is done
             if (tid == 0) issue_mma(0);
@@ -382,7 +388,6 @@ zwalk_kernel(const Tables* __restrict__ tab, const ZTables* __restrict__ zt, Ctr
             upk2(hh, Rlo, Rhi);
             const float R = fmaf(Rhi, m1[0], Rlo * m0[0]);
             // ---- a4: flag unless the block provably holds no configuration with E <= tauE ----
-            const float Lp = fmaf(lambda, (float)(tauE - Eh), lpb);
             const bool clear = (lg2f(R) + Lp < -Z_MARGIN) && (Lp <= Z_L_SAFE);
             unsigned hits = __ballot_sync(0xffffffffu, !clear);
             flagged += __popc(hits);

@@ -26,13 +26,21 @@ def test_reference_arm_prints_one_json_line():
 
 
 def test_stored_gpu_bench_line_has_the_contract_keys():
-    path = os.path.join(ROOT, "profiles", "r01_bench_full.txt")
+    path = os.path.join(ROOT, "profiles", "r02_bench_full.txt")
     line = [l for l in open(path) if l.startswith("{")][-1]
     d = json.loads(line)
-    assert BASE_KEYS | {"roofline", "clocks", "time_to_S_lowest_s", "per_config"} <= set(d)
+    assert BASE_KEYS | {"roofline", "roofline_packed16", "roofline_int32", "clocks", "time_to_S_lowest_s",
+                        "per_config"} <= set(d)
     r = d["roofline"]
     assert {"bound", "achieved", "peak", "unit", "frac", "traffic"} <= set(r)
-    assert r["bound"] == "alu" and abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-12 and 0 < r["frac"] < 1
+    assert r["bound"] == "tensor" and r["unit"] == "TFLOP/s" and r["kernel"] == "ising::zwalk_kernel"
+    assert abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-12 and 0 < r["frac"] < 1.2
+    # the GEMM work of the screen is 2 flop per configuration, counted over the kernel's own launches
+    assert abs(r["achieved"] - 2.0 * r["configs_per_s_in_kernel"] * 1e-12) < 1e-6 * r["achieved"]
+    for key in ("roofline_packed16", "roofline_int32"):
+        a = d[key]
+        assert a["bound"] == "alu" and abs(a["frac"] - a["achieved"] / a["peak"]) < 1e-12 and 0 < a["frac"] < 1
+        assert a["same_list_as_default_path"] is True
     assert d["n_gpus"] == 1 and d["steps"] >= 1 and d["warmup"] >= 3 and d["gpu_launches"] > 0
     assert d["clocks"]["reasons"] == [] or set(d["clocks"]["reasons"]) <= {"sw_power_cap"}
     assert d["e2e"]["h2d_bytes_per_step"] > 0 and d["e2e"]["d2h_bytes_per_step"] > 0

@@ -885,7 +885,7 @@ def test_first_calls_from_two_threads(B, tmp_path):
 
 # ---------- the tensor-core (tcgen05) screen of zscreen.cu, forced on at sizes the oracle reaches ----------
 @pytest.mark.parametrize("name", ["gauss24", "gauss26", "gauss27_h2", "int26", "sparse25", "mattis30", "wide24", "fields27",
-                                  "zero24"])
+                                  "zero24", "bigint26", "bigreal26"])
 def test_tensor_core_screen_small(B, name):
     """ISING_Z_MIN_LOG2 = 24 sends everything after the first eighth of the range through the partition-function
     screen (probe + bulk, or the packed kernel if the probe flags too much): the list must be the oracle's whatever
@@ -907,6 +907,19 @@ def test_tensor_core_screen_small(B, name):
         J, h = _wide_range_instance(24, 2424); S = 200
     elif name == "fields27":
         J, h = I.fields_only(27, seed=27); S = 50
+    elif name in ("bigint26", "bigreal26"):
+        # no couplings among the fourteen spins of the screen's block (lambda at its cap of 16 bits per grid unit) and
+        # strong fields: the log-domain offset L is a difference of terms of 2^25 bits and more, and a one-grid-unit
+        # error in it loses a state of an exact instance (integers of 20 bits: band = 0)
+        rng = np.random.default_rng(2626)
+        n = 26
+        J = np.triu(rng.integers(1, 1 << 17, (n, n)) * rng.choice([-1, 1], (n, n)), 1).astype(np.float64)
+        J[:14, :14] = 0.0
+        J = J + J.T
+        h = (rng.integers(1, 1 << 20, n) * rng.choice([-1, 1], n)).astype(np.float64)
+        if name == "bigreal26":
+            J = J * (1.0 + 2.0 ** -30); h = h * (1.0 - 2.0 ** -31)        # off every grid: guard band
+        S = 300
     else:
         J, h = np.zeros((24, 24)), np.zeros(24); S = 40
     q, e = _with_env({"ISING_Z_MIN_LOG2": 24}, lambda: gpu_lowest(B, J, h, S))
