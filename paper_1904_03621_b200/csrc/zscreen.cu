@@ -290,14 +290,17 @@ zwalk_kernel(const Tables* __restrict__ tab, const ZTables* __restrict__ zt, Ctr
             }
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");    // the row is read by the tensor core
         };
-        // One elected thread: D[buf] = A[buf] x T^T, eight K = 16 slices, completion signalled on mbar[buf].
+        // One elected thread: D[buf] = A[buf] x T^T, eight K = 16 slices, completion signalled on mbar[buf]. The two base
+        // descriptors are formed once (rebuilt per MMA they are a chain of ~17 uniform-datapath instructions each).
+        const unsigned long long desc_a0 = umma_desc(smem_u32(sA)), desc_b0 = umma_desc(smem_u32(sT));
         auto issue_mma = [&](int buf) {
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-            const unsigned a0 = smem_u32(sA) + (unsigned)buf * 32768u, b0 = smem_u32(sT);
 #pragma unroll
             for (int ks = 0; ks < 8; ++ks) {
-                const unsigned long long da = umma_desc(a0 + (unsigned)ks * 2u * Z_LBO);
-                const unsigned long long db = umma_desc(b0 + (unsigned)ks * 2u * Z_LBO);
+                // K slice ks starts 2 LBO bytes further on: + 16 in the descriptors' 16-byte address field (no carry out
+                // of its 14 bits: shared memory ends below 256 KB)
+                const unsigned long long da = desc_a0 + (unsigned long long)(ks * (2 * Z_LBO >> 4));
+                const unsigned long long db = desc_b0 + (unsigned long long)(ks * (2 * Z_LBO >> 4));
                 const unsigned acc = ks > 0 ? 1u : 0u;
                 asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
                              "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
