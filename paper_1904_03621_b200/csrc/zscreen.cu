@@ -139,6 +139,61 @@ __global__ void __launch_bounds__(1024) ztables_kernel(const Tables* __restrict_
     }
 }
 
+// ---- a flagged block of 2^14 configurations, formed exactly by the warp: sixteen blocks of 1024 (walk.cuh push_block).
+// P = the fourteen local fields of the flagged thread at the block's base state (block spins down), e0 = its grid
+// energy, both already broadcast to every lane. Setting block spin 10 + a raises the field of spin i by 2 Jq[i][10 + a],
+// so the lane's tables of the ten low spins and the base energy of sub-block `sub` follow from those of sub-block 0 by at
+// most four additions each (eqs. (2),(3)):
+//      E(q0 u A) = E(q0) - 2 sum_{a in A} Phi_a(q0) - 4 sum_{a<b in A} Jq_ab .
+// (Forming each sub-block from scratch -- every field re-summed over all N spins -- cost 75 us per flagged block, during
+// which the other three warps of the CTA wait at the step barrier: the tail of every launch of a few steps per CTA.) ----
+// Returns the number of sub-blocks that held a candidate; the threshold is re-read after those only.
+static __device__ __noinline__ unsigned form_flagged(const Tables* __restrict__ tab, Ctrl* __restrict__ ctrl,
+                                                     Entry* __restrict__ pool, unsigned* __restrict__ hist, const Plan& plan,
+                                                     const int (&P)[ZB], int e0, unsigned long long qh,
+                                                     unsigned long long& tau, int lane)
+{
+    static_assert(ZB == LOWBITS + 4, "sixteen sub-blocks");
+    const int* __restrict__ Jq = tab->Jq;
+    int vx0 = tab->QL[lane], ux0 = tab->QM[lane];
+#pragma unroll
+    for (int i = 0; i < LL; ++i) {
+        if (lane >> i & 1) { vx0 -= 2 * P[i]; ux0 -= 2 * P[LL + i]; }
+    }
+    int dvx[4], dux[4];
+#pragma unroll
+    for (int a = 0; a < 4; ++a) {
+        int sv = 0, su = 0;
+#pragma unroll
+        for (int i = 0; i < LL; ++i) {
+            if (lane >> i & 1) { sv += Jq[i * 64 + LOWBITS + a]; su += Jq[(LL + i) * 64 + LOWBITS + a]; }
+        }
+        dvx[a] = -4 * sv;
+        dux[a] = -4 * su;
+    }
+    unsigned n_true = 0;
+#pragma unroll 1
+    for (int sub = 0; sub < 16; ++sub) {
+        int vx = vx0, ux = ux0, eh = e0;
+#pragma unroll
+        for (int a = 0; a < 4; ++a) {
+            if (sub >> a & 1) {
+                vx += dvx[a];
+                ux += dux[a];
+                eh -= 2 * P[LOWBITS + a];
+#pragma unroll
+                for (int b = 0; b < a; ++b)
+                    if (sub >> b & 1) eh -= 4 * Jq[(LOWBITS + b) * 64 + LOWBITS + a];
+            }
+        }
+        if (push_block<false>(ctrl, pool, hist, plan, tab->C, qh + ((unsigned long long)sub << LOWBITS), vx, ux, eh, tau, lane)) {
+            ++n_true;
+            tau = ld_relaxed_u64(&ctrl->tau);
+        }
+    }
+    return n_true;
+}
+
 // ---- the screen kernel: one CTA of 128 threads per unit of 2^(21 + Lw) configurations ----
 __global__ void __launch_bounds__(Z_THREADS)
 zwalk_kernel(const Tables* __restrict__ tab, const ZTables* __restrict__ zt, Ctrl* __restrict__ ctrl,
@@ -198,6 +253,7 @@ zwalk_kernel(const Tables* __restrict__ tab, const ZTables* __restrict__ zt, Ctr
     const int* __restrict__ Jq = tab->Jq;
     const float lambda = zt->lambda, t0 = zt->t0;
     unsigned long long flagged = 0ull;
+    unsigned sub_true = 0;                                  // exactly formed blocks of 1024 that held a candidate
 
     if (!dead) {
         // ---- a2: base state. Warp: Phi_i(qW), E(qW) for the warp's first state; lane: its 5 lane bits on top ----
@@ -394,15 +450,30 @@ zwalk_kernel(const Tables* __restrict__ tab, const ZTables* __restrict__ zt, Ctr
             const bool clear = (lg2f(R) + Lp < -Z_MARGIN) && (Lp <= Z_L_SAFE);
             unsigned hits = __ballot_sync(0xffffffffu, !clear);
             flagged += __popc(hits);
-            while (hits) {
-                const int src = __ffs(hits) - 1;
-                hits &= hits - 1;
-                const unsigned gray = t ^ (t >> 1);
-                const unsigned long long qh = qW + ((unsigned long long)src << nlow) + ((unsigned long long)gray << ZB);
-#pragma unroll 1
-                for (int sub = 0; sub < (1 << (ZB - LOWBITS)); ++sub) {
-                    form_block<true>(tab, ctrl, pool, hist, plan, tab->C, qh + ((unsigned long long)sub << LOWBITS), 0, tau, lane);
-                    tau = ld_relaxed_u64(&ctrl->tau);
+            if (hits) {
+                // the fields of THIS step again (Phi already took the Gray step that follows it)
+                int Pt[ZB];
+                {
+                    const int4* dp = reinterpret_cast<const int4*>(sDPhi + k * 16);
+#pragma unroll
+                    for (int x = 0; x < 4; ++x) {
+                        const int4 d = dp[x];
+                        if (4 * x + 0 < ZB) Pt[4 * x + 0] = Phi[4 * x + 0] - (sb ? d.x : -d.x);
+                        if (4 * x + 1 < ZB) Pt[4 * x + 1] = Phi[4 * x + 1] - (sb ? d.y : -d.y);
+                        if (4 * x + 2 < ZB) Pt[4 * x + 2] = Phi[4 * x + 2] - (sb ? d.z : -d.z);
+                        if (4 * x + 3 < ZB) Pt[4 * x + 3] = Phi[4 * x + 3] - (sb ? d.w : -d.w);
+                    }
+                }
+                while (hits) {
+                    const int src = __ffs(hits) - 1;
+                    hits &= hits - 1;
+                    const unsigned gray = t ^ (t >> 1);
+                    const unsigned long long qh = qW + ((unsigned long long)src << nlow) + ((unsigned long long)gray << ZB);
+                    int P[ZB];
+#pragma unroll
+                    for (int i = 0; i < ZB; ++i) P[i] = __shfl_sync(0xffffffffu, Pt[i], src);
+                    const int e0 = __shfl_sync(0xffffffffu, Eh, src);
+                    sub_true += form_flagged(tab, ctrl, pool, hist, plan, P, e0, qh, tau, lane);
                 }
                 tauE = tau_energy(tau);
             }
@@ -417,7 +488,11 @@ zwalk_kernel(const Tables* __restrict__ tab, const ZTables* __restrict__ zt, Ctr
     // ---- unit complete ----
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
-    if (lane == 0 && flagged) atomicAdd(&ctrl->z_flagged, flagged);
+    if (lane == 0 && flagged) {
+        atomicAdd(&ctrl->z_flagged, flagged);
+        atomicAdd(&ctrl->hits, flagged << (ZB - LOWBITS));               // sixteen blocks of 1024 per flagged block ...
+        atomicAdd(&ctrl->false_hits, (flagged << (ZB - LOWBITS)) - sub_true);    // ... of which these held no candidate
+    }
     if (tid == 0) {
         atomicAdd(&ctrl->z_steps, (unsigned long long)Z_THREADS << (dead ? 0 : Lw));
         __threadfence();
