@@ -148,7 +148,10 @@ __device__ __forceinline__ unsigned push_block(Ctrl* __restrict__ ctrl, Entry* _
     const int tauE = tau_energy(tau);
     const unsigned qc = tau_qc(tau);
     const unsigned long long tauQ = qc == QC_NONE ? Q_MAX : plan.q_begin + ((unsigned long long)qc << plan.qshift);
-    const int loE = plan.loE;
+    // (the plan is reached through a reference here: read its fields once, not inside the loops)
+    const int loE = plan.loE, use_hist = plan.use_hist;
+    const unsigned long long q_end = plan.q_end;
+    const unsigned refresh_every = (unsigned)plan.refresh;
     const unsigned long long qs = qh + (unsigned)lane;
     const int v = vx + eh;
     unsigned mask = 0;
@@ -156,7 +159,7 @@ __device__ __forceinline__ unsigned push_block(Ctrl* __restrict__ ctrl, Entry* _
     for (int mid = 0; mid < NMID; ++mid) {
         const int e = v + sC[mid * NLO + lane] + __shfl_sync(0xffffffffu, ux, mid);
         const unsigned long long q = qs + ((unsigned)mid << LL);
-        const bool pass = (e < tauE || (e == tauE && q < tauQ)) && e >= loE && q < plan.q_end;
+        const bool pass = (e < tauE || (e == tauE && q < tauQ)) && e >= loE && q < q_end;
         mask |= pass ? (1u << mid) : 0u;
     }
     const int cnt = __popc(mask);
@@ -177,7 +180,7 @@ __device__ __forceinline__ unsigned push_block(Ctrl* __restrict__ ctrl, Entry* _
         if (total != 0 && ld_relaxed_u32(&ctrl->pool_overflow) == 0u) {
             slot = atomicAdd(&ctrl->count, total);
             if (slot + total > POOL_CAP) atomicExch(&ctrl->pool_overflow, 1u);
-            refresh = plan.use_hist && (slot / (unsigned)plan.refresh != (slot + total) / (unsigned)plan.refresh);
+            refresh = use_hist && (slot / refresh_every != (slot + total) / refresh_every);
         }
     }
     if (total == 0) return 0u;                                   // a false hit of the screen
@@ -195,7 +198,7 @@ __device__ __forceinline__ unsigned push_block(Ctrl* __restrict__ ctrl, Entry* _
                 en.key = key_from_i32(e);
                 en.q = qs + ((unsigned)mid << LL);
                 pool[slot] = en;
-                if (plan.use_hist) {
+                if (use_hist) {
                     const int b = hist_bin(e, Wq, hs);
                     atomicAdd(hist + HIST_COARSE + b, 1u);
                     atomicAdd(hist + (b >> 8), 1u);

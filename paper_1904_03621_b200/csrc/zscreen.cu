@@ -150,11 +150,17 @@ __global__ void __launch_bounds__(1024) ztables_kernel(const Tables* __restrict_
 // Returns the number of sub-blocks that held a candidate; the threshold is re-read after those only.
 static __device__ __noinline__ unsigned form_flagged(const Tables* __restrict__ tab, Ctrl* __restrict__ ctrl,
                                                      Entry* __restrict__ pool, unsigned* __restrict__ hist, const Plan& plan,
-                                                     const int (&P)[ZB], int e0, unsigned long long qh,
-                                                     unsigned long long& tau, int lane)
+                                                     const int* sC, const int (&Pin)[ZB], int e0, unsigned long long qh,
+                                                     unsigned long long& tau_io, int lane)
 {
     static_assert(ZB == LOWBITS + 4, "sixteen sub-blocks");
     const int* __restrict__ Jq = tab->Jq;
+    // reference arguments of an out-of-line function live in local memory, and with no L1 left on the SM every access
+    // to it is an L2 round trip: read them once, keep registers
+    int P[ZB];
+#pragma unroll
+    for (int i = 0; i < ZB; ++i) P[i] = Pin[i];
+    unsigned long long tau = tau_io;
     int vx0 = tab->QL[lane], ux0 = tab->QM[lane];
 #pragma unroll
     for (int i = 0; i < LL; ++i) {
@@ -171,6 +177,11 @@ static __device__ __noinline__ unsigned form_flagged(const Tables* __restrict__ 
         dvx[a] = -4 * sv;
         dux[a] = -4 * su;
     }
+    int jp[4][4];                                           // couplings among the four upper block spins (read once: L2)
+#pragma unroll
+    for (int a = 0; a < 4; ++a)
+#pragma unroll
+        for (int b = 0; b < a; ++b) jp[b][a] = 4 * Jq[(LOWBITS + b) * 64 + LOWBITS + a];
     unsigned n_true = 0;
 #pragma unroll 1
     for (int sub = 0; sub < 16; ++sub) {
@@ -183,14 +194,15 @@ static __device__ __noinline__ unsigned form_flagged(const Tables* __restrict__ 
                 eh -= 2 * P[LOWBITS + a];
 #pragma unroll
                 for (int b = 0; b < a; ++b)
-                    if (sub >> b & 1) eh -= 4 * Jq[(LOWBITS + b) * 64 + LOWBITS + a];
+                    if (sub >> b & 1) eh -= jp[b][a];
             }
         }
-        if (push_block<false>(ctrl, pool, hist, plan, tab->C, qh + ((unsigned long long)sub << LOWBITS), vx, ux, eh, tau, lane)) {
+        if (push_block<false>(ctrl, pool, hist, plan, sC, qh + ((unsigned long long)sub << LOWBITS), vx, ux, eh, tau, lane)) {
             ++n_true;
             tau = ld_relaxed_u64(&ctrl->tau);
         }
     }
+    tau_io = tau;
     return n_true;
 }
 
@@ -451,6 +463,18 @@ zwalk_kernel(const Tables* __restrict__ tab, const ZTables* __restrict__ zt, Ctr
             unsigned hits = __ballot_sync(0xffffffffu, !clear);
             flagged += __popc(hits);
             if (hits) {
+                // The C table of the 1024-configuration blocks (4 KB) goes to shared memory first: with three CTAs of 75 KB
+                // the SM has no L1 left, and every one of the 16 x 32 table reads of a flagged block would be an L2 round
+                // trip (measured: 70 000 clocks per flagged block, the whole CTA waiting). The warp's own eight row groups
+                // of the A tile (8 KB, contiguous in the canonical layout) are free here: the MMAs of this step are
+                // complete and only this warp writes these rows again, in the next row generation.
+                int* const myC = reinterpret_cast<int*>(sA + (unsigned)warp * 8192u);
+                {
+                    const int4* __restrict__ src4 = reinterpret_cast<const int4*>(tab->C);
+#pragma unroll
+                    for (int i = 0; i < (NMID * NLO / 4) / 32; ++i) reinterpret_cast<int4*>(myC)[i * 32 + lane] = src4[i * 32 + lane];
+                    __syncwarp();
+                }
                 // the fields of THIS step again (Phi already took the Gray step that follows it)
                 int Pt[ZB];
                 {
@@ -473,7 +497,7 @@ zwalk_kernel(const Tables* __restrict__ tab, const ZTables* __restrict__ zt, Ctr
 #pragma unroll
                     for (int i = 0; i < ZB; ++i) P[i] = __shfl_sync(0xffffffffu, Pt[i], src);
                     const int e0 = __shfl_sync(0xffffffffu, Eh, src);
-                    sub_true += form_flagged(tab, ctrl, pool, hist, plan, P, e0, qh, tau, lane);
+                    sub_true += form_flagged(tab, ctrl, pool, hist, plan, myC, P, e0, qh, tau, lane);
                 }
                 tauE = tau_energy(tau);
             }
