@@ -143,7 +143,7 @@ __device__ __forceinline__ int warp_fields(const Tables* __restrict__ tab, int N
 template <bool COUNT>
 __device__ __forceinline__ unsigned push_block(Ctrl* __restrict__ ctrl, Entry* __restrict__ pool, unsigned* __restrict__ hist,
                                            const Plan& plan, const int* sC, unsigned long long qh, int vx, int ux, int eh,
-                                           unsigned long long tau, int lane)
+                                           unsigned long long tau, int lane, unsigned refresh_override = 0u)
 {
     const int tauE = tau_energy(tau);
     const unsigned qc = tau_qc(tau);
@@ -151,7 +151,8 @@ __device__ __forceinline__ unsigned push_block(Ctrl* __restrict__ ctrl, Entry* _
     // (the plan is reached through a reference here: read its fields once, not inside the loops)
     const int loE = plan.loE, use_hist = plan.use_hist;
     const unsigned long long q_end = plan.q_end;
-    const unsigned refresh_every = (unsigned)plan.refresh;
+    // threshold-free blocks push all their 1024 configurations: one refresh per block there, not one per plan.refresh
+    const unsigned refresh_every = refresh_override ? refresh_override : (unsigned)plan.refresh;
     const unsigned long long qs = qh + (unsigned)lane;
     const int v = vx + eh;
     unsigned mask = 0;
@@ -192,19 +193,27 @@ __device__ __forceinline__ unsigned push_block(Ctrl* __restrict__ ctrl, Entry* _
     const int hs = ctrl->hist_shift;
     for (int mid = 0; mid < NMID; ++mid) {
         const int e = v + sC[mid * NLO + lane] + __shfl_sync(0xffffffffu, ux, mid);
-        if (mask >> mid & 1u) {
+        const bool mine = (mask >> mid & 1u) != 0u;
+        const unsigned act = __ballot_sync(0xffffffffu, mine);
+        if (mine) {
             if (slot < POOL_CAP) {
                 Entry en;
                 en.key = key_from_i32(e);
                 en.q = qs + ((unsigned)mid << LL);
                 pool[slot] = en;
-                if (use_hist) {
-                    const int b = hist_bin(e, Wq, hs);
-                    atomicAdd(hist + HIST_COARSE + b, 1u);
-                    atomicAdd(hist + (b >> 8), 1u);
-                }
             }
             ++slot;
+            if (use_hist) {
+                // lanes of one bin count together: on degenerate instances (a few dozen distinct energies) thousands of
+                // candidates of the threshold-free first blocks would otherwise queue on the same two counters
+                const int b = hist_bin(e, Wq, hs);
+                const unsigned peers = __match_any_sync(act, b);
+                if ((unsigned)lane == (unsigned)(__ffs(peers) - 1)) {
+                    const unsigned n = (unsigned)__popc(peers);
+                    atomicAdd(hist + HIST_COARSE + b, n);
+                    atomicAdd(hist + (b >> 8), n);
+                }
+            }
         }
     }
     if (refresh) {
@@ -221,7 +230,8 @@ __device__ __forceinline__ unsigned push_block(Ctrl* __restrict__ ctrl, Entry* _
 template <bool FROM_SCRATCH>
 __device__ __noinline__ void form_block(const Tables* __restrict__ tab, Ctrl* __restrict__ ctrl,
                                         Entry* __restrict__ pool, unsigned* __restrict__ hist, const Plan& plan,
-                                        const int* sC, unsigned long long qh, int eh, unsigned long long tau, int lane)
+                                        const int* sC, unsigned long long qh, int eh, unsigned long long tau, int lane,
+                                        unsigned refresh_override = 0u)
 {
     const int N = plan.N;
     int vx = tab->QL[lane], ux = tab->QM[lane];
@@ -248,7 +258,7 @@ __device__ __noinline__ void form_block(const Tables* __restrict__ tab, Ctrl* __
             else        { if (lane >> (i - LL) & 1) ux -= 2 * f; }
         }
     }
-    push_block<true>(ctrl, pool, hist, plan, sC, qh, vx, ux, eh, tau, lane);
+    push_block<true>(ctrl, pool, hist, plan, sC, qh, vx, ux, eh, tau, lane, refresh_override);
 }
 
 // The persistent kernel. INNER supplies the per-thread tables of the 1024-configuration block and its screen:
@@ -306,7 +316,7 @@ walk_kernel(const Tables* __restrict__ tab, Ctrl* __restrict__ ctrl, Entry* __re
 
         if (unit_bits == LOWBITS) {
             // ---- a2': one block formed exactly, nothing screened (the threshold does not exist yet) ----
-            form_block<true>(tab, ctrl, pool, hist, plan, sC, qW, 0, tau, lane);
+            form_block<true>(tab, ctrl, pool, hist, plan, sC, qW, 0, tau, lane, need == 0ull ? (unsigned)(NLO * NMID) : 0u);
         } else {
             const int Lw = unit_bits - MIN_CHUNK_BITS;
             const int nlow = LOWBITS + Lw;
