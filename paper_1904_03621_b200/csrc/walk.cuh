@@ -136,102 +136,12 @@ __device__ __forceinline__ int warp_fields(const Tables* __restrict__ tab, int N
 }
 
 // a4, second half: the whole warp forms the 1024 energies of one block exactly (int32 grid units) and pushes the
-// survivors. qh = the block's state with lo and mid bits zero, eh = its grid energy; lane l holds the block's tables
-// vx = V[lo = l], ux = U[mid = l] (common.cuh vocabulary). Two passes: mark the survivors, reserve their pool slots with
-// ONE atomic per block, then write. Returns the number of survivors. COUNT: bump the hit statistics in Ctrl here (the
-// tensor-core screen counts in registers instead: every global round trip of a flagged block is paid by a whole CTA).
-template <bool COUNT>
-__device__ __forceinline__ unsigned push_block(Ctrl* __restrict__ ctrl, Entry* __restrict__ pool, unsigned* __restrict__ hist,
-                                           const Plan& plan, const int* sC, unsigned long long qh, int vx, int ux, int eh,
-                                           unsigned long long tau, int lane, unsigned refresh_override = 0u)
-{
-    const int tauE = tau_energy(tau);
-    const unsigned qc = tau_qc(tau);
-    const unsigned long long tauQ = qc == QC_NONE ? Q_MAX : plan.q_begin + ((unsigned long long)qc << plan.qshift);
-    // (the plan is reached through a reference here: read its fields once, not inside the loops)
-    const int loE = plan.loE, use_hist = plan.use_hist;
-    const unsigned long long q_end = plan.q_end;
-    // threshold-free blocks push all their 1024 configurations: one refresh per block there, not one per plan.refresh
-    const unsigned refresh_every = refresh_override ? refresh_override : (unsigned)plan.refresh;
-    const unsigned long long qs = qh + (unsigned)lane;
-    const int v = vx + eh;
-    unsigned mask = 0;
-#pragma unroll 8
-    for (int mid = 0; mid < NMID; ++mid) {
-        const int e = v + sC[mid * NLO + lane] + __shfl_sync(0xffffffffu, ux, mid);
-        const unsigned long long q = qs + ((unsigned)mid << LL);
-        const bool pass = (e < tauE || (e == tauE && q < tauQ)) && e >= loE && q < q_end;
-        mask |= pass ? (1u << mid) : 0u;
-    }
-    const int cnt = __popc(mask);
-    int incl = cnt;
-#pragma unroll
-    for (int d = 1; d < 32; d <<= 1) {
-        const int n = __shfl_up_sync(0xffffffffu, incl, d);
-        if (lane >= d) incl += n;
-    }
-    const unsigned total = (unsigned)__shfl_sync(0xffffffffu, incl, 31);
-    unsigned slot = POOL_CAP;
-    int refresh = 0;
-    if (lane == 0) {
-        if (COUNT) {
-            atomicAdd(&ctrl->hits, 1ull);
-            if (total == 0) atomicAdd(&ctrl->false_hits, 1ull);
-        }
-        if (total != 0 && ld_relaxed_u32(&ctrl->pool_overflow) == 0u) {
-            slot = atomicAdd(&ctrl->count, total);
-            if (slot + total > POOL_CAP) atomicExch(&ctrl->pool_overflow, 1u);
-            refresh = use_hist && (slot / refresh_every != (slot + total) / refresh_every);
-        }
-    }
-    if (total == 0) return 0u;                                   // a false hit of the screen
-    slot = __shfl_sync(0xffffffffu, slot, 0);
-    refresh = __shfl_sync(0xffffffffu, refresh, 0);
-    if (slot >= POOL_CAP) return total;                          // the pool is full: the run is void (sticky flag)
-    slot += (unsigned)(incl - cnt);
-    const long long Wq = ctrl->Wq;
-    const int hs = ctrl->hist_shift;
-    for (int mid = 0; mid < NMID; ++mid) {
-        const int e = v + sC[mid * NLO + lane] + __shfl_sync(0xffffffffu, ux, mid);
-        const bool mine = (mask >> mid & 1u) != 0u;
-        const unsigned act = __ballot_sync(0xffffffffu, mine);
-        if (mine) {
-            if (slot < POOL_CAP) {
-                Entry en;
-                en.key = key_from_i32(e);
-                en.q = qs + ((unsigned)mid << LL);
-                pool[slot] = en;
-            }
-            ++slot;
-            if (use_hist) {
-                // lanes of one bin count together: on degenerate instances (a few dozen distinct energies) thousands of
-                // candidates of the threshold-free first blocks would otherwise queue on the same two counters
-                const int b = hist_bin(e, Wq, hs);
-                const unsigned peers = __match_any_sync(act, b);
-                if ((unsigned)lane == (unsigned)(__ffs(peers) - 1)) {
-                    const unsigned n = (unsigned)__popc(peers);
-                    atomicAdd(hist + HIST_COARSE + b, n);
-                    atomicAdd(hist + (b >> 8), n);
-                }
-            }
-        }
-    }
-    if (refresh) {
-        __threadfence();
-        __syncwarp();
-        refresh_tau(ctrl, hist, plan, lane);
-    }
-    return total;
-}
-
-// a4, second half, for the ALU kernels: the block's tables from its ten local fields -- computed from scratch
-// (FROM_SCRATCH: fields and energy of qh by the warp) or, with eh given, re-summed by the warp -- then push_block.
+// survivors. qh = the block's state with lo and mid bits zero, eh = its grid energy (FROM_SCRATCH: computed here).
 // Kept out of line so that its registers do not weigh on the enumeration loop.
 template <bool FROM_SCRATCH>
 __device__ __noinline__ void form_block(const Tables* __restrict__ tab, Ctrl* __restrict__ ctrl,
                                         Entry* __restrict__ pool, unsigned* __restrict__ hist, const Plan& plan,
-                                        const int* sC, unsigned long long qh, int eh, unsigned long long tau, int lane,
-                                        unsigned refresh_override = 0u)
+                                        const int* sC, unsigned long long qh, int eh, unsigned long long tau, int lane)
 {
     const int N = plan.N;
     int vx = tab->QL[lane], ux = tab->QM[lane];
@@ -258,7 +168,68 @@ __device__ __noinline__ void form_block(const Tables* __restrict__ tab, Ctrl* __
             else        { if (lane >> (i - LL) & 1) ux -= 2 * f; }
         }
     }
-    push_block<true>(ctrl, pool, hist, plan, sC, qh, vx, ux, eh, tau, lane, refresh_override);
+    const int tauE = tau_energy(tau);
+    const unsigned qc = tau_qc(tau);
+    const unsigned long long tauQ = qc == QC_NONE ? Q_MAX : plan.q_begin + ((unsigned long long)qc << plan.qshift);
+    const int loE = plan.loE;
+    const unsigned long long qs = qh + (unsigned)lane;
+    const int v = vx + eh;
+    // two passes: mark the survivors, reserve their pool slots with ONE atomic per block, then write
+    unsigned mask = 0;
+    for (int mid = 0; mid < NMID; ++mid) {
+        const int e = v + sC[mid * NLO + lane] + __shfl_sync(0xffffffffu, ux, mid);
+        const unsigned long long q = qs + ((unsigned)mid << LL);
+        const bool pass = (e < tauE || (e == tauE && q < tauQ)) && e >= loE && q < plan.q_end;
+        mask |= pass ? (1u << mid) : 0u;
+    }
+    const int cnt = __popc(mask);
+    int incl = cnt;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const int n = __shfl_up_sync(0xffffffffu, incl, d);
+        if (lane >= d) incl += n;
+    }
+    const unsigned total = (unsigned)__shfl_sync(0xffffffffu, incl, 31);
+    unsigned slot = POOL_CAP;
+    int refresh = 0;
+    if (lane == 0) {
+        atomicAdd(&ctrl->hits, 1ull);
+        if (total == 0) atomicAdd(&ctrl->false_hits, 1ull);
+        else if (ld_relaxed_u32(&ctrl->pool_overflow) == 0u) {
+            slot = atomicAdd(&ctrl->count, total);
+            if (slot + total > POOL_CAP) atomicExch(&ctrl->pool_overflow, 1u);
+            refresh = plan.use_hist && (slot / (unsigned)plan.refresh != (slot + total) / (unsigned)plan.refresh);
+        }
+    }
+    if (total == 0) return;                                      // a false hit of the screen
+    slot = __shfl_sync(0xffffffffu, slot, 0);
+    refresh = __shfl_sync(0xffffffffu, refresh, 0);
+    if (slot >= POOL_CAP) return;                                // the pool is full: the run is void (sticky flag)
+    slot += (unsigned)(incl - cnt);
+    const long long Wq = ctrl->Wq;
+    const int hs = ctrl->hist_shift;
+    for (int mid = 0; mid < NMID; ++mid) {
+        const int e = v + sC[mid * NLO + lane] + __shfl_sync(0xffffffffu, ux, mid);
+        if (mask >> mid & 1u) {
+            if (slot < POOL_CAP) {
+                Entry en;
+                en.key = key_from_i32(e);
+                en.q = qs + ((unsigned)mid << LL);
+                pool[slot] = en;
+                if (plan.use_hist) {
+                    const int b = hist_bin(e, Wq, hs);
+                    atomicAdd(hist + HIST_COARSE + b, 1u);
+                    atomicAdd(hist + (b >> 8), 1u);
+                }
+            }
+            ++slot;
+        }
+    }
+    if (refresh) {
+        __threadfence();
+        __syncwarp();
+        refresh_tau(ctrl, hist, plan, lane);
+    }
 }
 
 // The persistent kernel. INNER supplies the per-thread tables of the 1024-configuration block and its screen:
@@ -316,7 +287,7 @@ walk_kernel(const Tables* __restrict__ tab, Ctrl* __restrict__ ctrl, Entry* __re
 
         if (unit_bits == LOWBITS) {
             // ---- a2': one block formed exactly, nothing screened (the threshold does not exist yet) ----
-            form_block<true>(tab, ctrl, pool, hist, plan, sC, qW, 0, tau, lane, need == 0ull ? (unsigned)(NLO * NMID) : 0u);
+            form_block<true>(tab, ctrl, pool, hist, plan, sC, qW, 0, tau, lane);
         } else {
             const int Lw = unit_bits - MIN_CHUNK_BITS;
             const int nlow = LOWBITS + Lw;

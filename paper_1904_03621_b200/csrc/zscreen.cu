@@ -139,7 +139,93 @@ __global__ void __launch_bounds__(1024) ztables_kernel(const Tables* __restrict_
     }
 }
 
-// ---- a flagged block of 2^14 configurations, formed exactly by the warp: sixteen blocks of 1024 (walk.cuh push_block).
+// a4, second half: the whole warp forms the 1024 energies of one block exactly (int32 grid units) and pushes the
+// survivors. qh = the block's state with lo and mid bits zero, eh = its grid energy; lane l holds the block's tables
+// vx = V[lo = l], ux = U[mid = l] (common.cuh vocabulary). Two passes: mark the survivors, reserve their pool slots with
+// ONE atomic per block, then write. Returns the number of survivors. (walk.cuh form_block is the ALU kernels' version of
+// the same steps; this one counts the hit statistics in registers -- every global round trip of a flagged block is paid
+// by a whole CTA -- reads the plan's fields once, and updates the histogram once per bin and warp. It is kept apart so
+// that the register allocation of the ALU kernels' loop, which ptxas ties to the code of the function it calls, stays
+// the conflict-free one: enumerate16.cu header.)
+__device__ __forceinline__ unsigned push_block(Ctrl* __restrict__ ctrl, Entry* __restrict__ pool, unsigned* __restrict__ hist,
+                                           const Plan& plan, const int* sC, unsigned long long qh, int vx, int ux, int eh,
+                                           unsigned long long tau, int lane)
+{
+    const int tauE = tau_energy(tau);
+    const unsigned qc = tau_qc(tau);
+    const unsigned long long tauQ = qc == QC_NONE ? Q_MAX : plan.q_begin + ((unsigned long long)qc << plan.qshift);
+    // (the plan is reached through a reference here: read its fields once, not inside the loops)
+    const int loE = plan.loE, use_hist = plan.use_hist;
+    const unsigned long long q_end = plan.q_end;
+    const unsigned refresh_every = (unsigned)plan.refresh;
+    const unsigned long long qs = qh + (unsigned)lane;
+    const int v = vx + eh;
+    unsigned mask = 0;
+#pragma unroll 8
+    for (int mid = 0; mid < NMID; ++mid) {
+        const int e = v + sC[mid * NLO + lane] + __shfl_sync(0xffffffffu, ux, mid);
+        const unsigned long long q = qs + ((unsigned)mid << LL);
+        const bool pass = (e < tauE || (e == tauE && q < tauQ)) && e >= loE && q < q_end;
+        mask |= pass ? (1u << mid) : 0u;
+    }
+    const int cnt = __popc(mask);
+    int incl = cnt;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const int n = __shfl_up_sync(0xffffffffu, incl, d);
+        if (lane >= d) incl += n;
+    }
+    const unsigned total = (unsigned)__shfl_sync(0xffffffffu, incl, 31);
+    unsigned slot = POOL_CAP;
+    int refresh = 0;
+    if (lane == 0) {
+        if (total != 0 && ld_relaxed_u32(&ctrl->pool_overflow) == 0u) {
+            slot = atomicAdd(&ctrl->count, total);
+            if (slot + total > POOL_CAP) atomicExch(&ctrl->pool_overflow, 1u);
+            refresh = use_hist && (slot / refresh_every != (slot + total) / refresh_every);
+        }
+    }
+    if (total == 0) return 0u;                                   // a false hit of the screen
+    slot = __shfl_sync(0xffffffffu, slot, 0);
+    refresh = __shfl_sync(0xffffffffu, refresh, 0);
+    if (slot >= POOL_CAP) return total;                          // the pool is full: the run is void (sticky flag)
+    slot += (unsigned)(incl - cnt);
+    const long long Wq = ctrl->Wq;
+    const int hs = ctrl->hist_shift;
+    for (int mid = 0; mid < NMID; ++mid) {
+        const int e = v + sC[mid * NLO + lane] + __shfl_sync(0xffffffffu, ux, mid);
+        const bool mine = (mask >> mid & 1u) != 0u;
+        const unsigned act = __ballot_sync(0xffffffffu, mine);
+        if (mine) {
+            if (slot < POOL_CAP) {
+                Entry en;
+                en.key = key_from_i32(e);
+                en.q = qs + ((unsigned)mid << LL);
+                pool[slot] = en;
+            }
+            ++slot;
+            if (use_hist) {
+                // lanes of one bin count together: on degenerate instances (a few dozen distinct energies) thousands of
+                // candidates of the threshold-free first blocks would otherwise queue on the same two counters
+                const int b = hist_bin(e, Wq, hs);
+                const unsigned peers = __match_any_sync(act, b);
+                if ((unsigned)lane == (unsigned)(__ffs(peers) - 1)) {
+                    const unsigned n = (unsigned)__popc(peers);
+                    atomicAdd(hist + HIST_COARSE + b, n);
+                    atomicAdd(hist + (b >> 8), n);
+                }
+            }
+        }
+    }
+    if (refresh) {
+        __threadfence();
+        __syncwarp();
+        refresh_tau(ctrl, hist, plan, lane);
+    }
+    return total;
+}
+
+// ---- a flagged block of 2^14 configurations, formed exactly by the warp: sixteen blocks of 1024 (push_block above).
 // P = the fourteen local fields of the flagged thread at the block's base state (block spins down), e0 = its grid
 // energy, both already broadcast to every lane. Setting block spin 10 + a raises the field of spin i by 2 Jq[i][10 + a],
 // so the lane's tables of the ten low spins and the base energy of sub-block `sub` follow from those of sub-block 0 by at
@@ -148,7 +234,7 @@ __global__ void __launch_bounds__(1024) ztables_kernel(const Tables* __restrict_
 // (Forming each sub-block from scratch -- every field re-summed over all N spins -- cost 75 us per flagged block, during
 // which the other three warps of the CTA wait at the step barrier: the tail of every launch of a few steps per CTA.) ----
 // Returns the number of sub-blocks that held a candidate; the threshold is re-read after those only.
-static __device__ __noinline__ unsigned form_flagged(const Tables* __restrict__ tab, Ctrl* __restrict__ ctrl,
+static __device__ __forceinline__ unsigned form_flagged(const Tables* __restrict__ tab, Ctrl* __restrict__ ctrl,
                                                      Entry* __restrict__ pool, unsigned* __restrict__ hist, const Plan& plan,
                                                      const int* sC, const int (&Pin)[ZB], int e0, unsigned long long qh,
                                                      unsigned long long& tau_io, int lane)
@@ -197,10 +283,46 @@ static __device__ __noinline__ unsigned form_flagged(const Tables* __restrict__ 
                     if (sub >> b & 1) eh -= jp[b][a];
             }
         }
-        if (push_block<false>(ctrl, pool, hist, plan, sC, qh + ((unsigned long long)sub << LOWBITS), vx, ux, eh, tau, lane)) {
+        if (push_block(ctrl, pool, hist, plan, sC, qh + ((unsigned long long)sub << LOWBITS), vx, ux, eh, tau, lane)) {
             ++n_true;
             tau = ld_relaxed_u64(&ctrl->tau);
         }
+    }
+    tau_io = tau;
+    return n_true;
+}
+
+// ---- all flagged blocks of one warp and step. myC: 4 KB of shared memory for the C table of the 1024-configuration
+// blocks -- with three CTAs of 75 KB the SM has no L1 left, and every one of the 16 x 32 table reads of a flagged block
+// would be an L2 round trip (measured: 70 000 clocks per flagged block, the whole CTA waiting); the warp's own eight row
+// groups of the A tile (8 KB, contiguous in the canonical layout) are free here: the MMAs of this step are complete and
+// only this warp writes these rows again, in the next row generation. Phi has already taken the Gray step that follows
+// this block (row dphi of the step table, direction sb): the fields of THIS step are recovered first. ----
+static __device__ __noinline__ unsigned handle_flagged(const Tables* __restrict__ tab, Ctrl* __restrict__ ctrl,
+                                                       Entry* __restrict__ pool, unsigned* __restrict__ hist, const Plan& plan,
+                                                       int* myC, const int* dphi, int sb, const int (&PhiNext)[ZB], int Eh,
+                                                       unsigned hits, unsigned long long q_step, int nlow,
+                                                       unsigned long long& tau_io, int lane)
+{
+    {
+        const int4* __restrict__ src4 = reinterpret_cast<const int4*>(tab->C);
+#pragma unroll
+        for (int i = 0; i < (NMID * NLO / 4) / 32; ++i) reinterpret_cast<int4*>(myC)[i * 32 + lane] = src4[i * 32 + lane];
+        __syncwarp();
+    }
+    int Pt[ZB];
+#pragma unroll
+    for (int i = 0; i < ZB; ++i) Pt[i] = PhiNext[i] - (sb ? dphi[i] : -dphi[i]);
+    unsigned long long tau = tau_io;
+    unsigned n_true = 0;
+    while (hits) {
+        const int src = __ffs(hits) - 1;
+        hits &= hits - 1;
+        int P[ZB];
+#pragma unroll
+        for (int i = 0; i < ZB; ++i) P[i] = __shfl_sync(0xffffffffu, Pt[i], src);
+        const int e0 = __shfl_sync(0xffffffffu, Eh, src);
+        n_true += form_flagged(tab, ctrl, pool, hist, plan, myC, P, e0, q_step + ((unsigned long long)src << nlow), tau, lane);
     }
     tau_io = tau;
     return n_true;
@@ -463,42 +585,10 @@ zwalk_kernel(const Tables* __restrict__ tab, const ZTables* __restrict__ zt, Ctr
             unsigned hits = __ballot_sync(0xffffffffu, !clear);
             flagged += __popc(hits);
             if (hits) {
-                // The C table of the 1024-configuration blocks (4 KB) goes to shared memory first: with three CTAs of 75 KB
-                // the SM has no L1 left, and every one of the 16 x 32 table reads of a flagged block would be an L2 round
-                // trip (measured: 70 000 clocks per flagged block, the whole CTA waiting). The warp's own eight row groups
-                // of the A tile (8 KB, contiguous in the canonical layout) are free here: the MMAs of this step are
-                // complete and only this warp writes these rows again, in the next row generation.
-                int* const myC = reinterpret_cast<int*>(sA + (unsigned)warp * 8192u);
-                {
-                    const int4* __restrict__ src4 = reinterpret_cast<const int4*>(tab->C);
-#pragma unroll
-                    for (int i = 0; i < (NMID * NLO / 4) / 32; ++i) reinterpret_cast<int4*>(myC)[i * 32 + lane] = src4[i * 32 + lane];
-                    __syncwarp();
-                }
-                // the fields of THIS step again (Phi already took the Gray step that follows it)
-                int Pt[ZB];
-                {
-                    const int4* dp = reinterpret_cast<const int4*>(sDPhi + k * 16);
-#pragma unroll
-                    for (int x = 0; x < 4; ++x) {
-                        const int4 d = dp[x];
-                        if (4 * x + 0 < ZB) Pt[4 * x + 0] = Phi[4 * x + 0] - (sb ? d.x : -d.x);
-                        if (4 * x + 1 < ZB) Pt[4 * x + 1] = Phi[4 * x + 1] - (sb ? d.y : -d.y);
-                        if (4 * x + 2 < ZB) Pt[4 * x + 2] = Phi[4 * x + 2] - (sb ? d.z : -d.z);
-                        if (4 * x + 3 < ZB) Pt[4 * x + 3] = Phi[4 * x + 3] - (sb ? d.w : -d.w);
-                    }
-                }
-                while (hits) {
-                    const int src = __ffs(hits) - 1;
-                    hits &= hits - 1;
-                    const unsigned gray = t ^ (t >> 1);
-                    const unsigned long long qh = qW + ((unsigned long long)src << nlow) + ((unsigned long long)gray << ZB);
-                    int P[ZB];
-#pragma unroll
-                    for (int i = 0; i < ZB; ++i) P[i] = __shfl_sync(0xffffffffu, Pt[i], src);
-                    const int e0 = __shfl_sync(0xffffffffu, Eh, src);
-                    sub_true += form_flagged(tab, ctrl, pool, hist, plan, myC, P, e0, qh, tau, lane);
-                }
+                // (out of line: the registers of this rare path must not weigh on the loop)
+                sub_true += handle_flagged(tab, ctrl, pool, hist, plan, reinterpret_cast<int*>(sA + (unsigned)warp * 8192u),
+                                           sDPhi + k * 16, sb, Phi, Eh, hits,
+                                           qW + ((unsigned long long)(t ^ (t >> 1)) << ZB), nlow, tau, lane);
                 tauE = tau_energy(tau);
             }
             // ---- move on to step t + 1 ----

@@ -107,3 +107,27 @@ def test_product_does_not_import_oracle():
         if fn.endswith((".py", ".c", ".h")):
             text = open(os.path.join(ROOT, "oracle", fn)).read()
             assert not bad_in_oracle.search(text), fn
+
+
+def test_packed_kernel_register_allocation(lib):
+    """The packed kernel's rate depends on ptxas finding an allocation in which the three sources of every packed
+    add-min sit in different register banks, and on the loop using no local memory (csrc/enumerate16.cu header; a change
+    in a function the loop calls has cost 7 % before). Checked on the built library with cuobjdump; it also proves the
+    tensor-core kernel really issues tcgen05 MMAs and TMEM loads (SASS UTCHMMA / LDTM)."""
+    import subprocess
+    from paper_1904_03621_b200 import binding
+    cuobjdump = shutil.which("cuobjdump") or "/usr/local/cuda/bin/cuobjdump"
+    sass = subprocess.run([cuobjdump, "-sass", binding.LIB_PATH], capture_output=True, text=True, timeout=600).stdout
+    funcs = re.split(r"\n\s*Function : ", sass)
+    walk16 = [f for f in funcs if f.startswith("_ZN5ising11walk_kernelINS_7Inner16")]
+    zwalk = [f for f in funcs if f.startswith("_ZN5ising12zwalk_kernel")]
+    assert len(walk16) == 1 and len(zwalk) == 1
+    mins = same_bank = 0
+    for m in re.finditer(r"(?:VIADDMNMX|VIMNMX3)\.U16x2\s+R\d+, R(\d+)(?:\.reuse)?, R(\d+)(?:\.reuse)?, R(\d+)", walk16[0]):
+        regs = [int(g) for g in m.groups()]
+        mins += 1
+        same_bank += len(set(regs)) == 3 and len({r & 1 for r in regs}) == 1
+    assert mins >= 400, mins
+    assert same_bank <= 6, f"{same_bank} of {mins} packed add-mins read three registers of one bank"
+    assert not re.search(r"\b(LDL|STL)\b", walk16[0]), "the packed kernel spills"
+    assert zwalk[0].count("UTCHMMA") >= 8 and "LDTM" in zwalk[0]
