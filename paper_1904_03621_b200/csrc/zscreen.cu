@@ -329,7 +329,7 @@ static __device__ __noinline__ unsigned handle_flagged(const Tables* __restrict_
 }
 
 // ---- the screen kernel: one CTA of 128 threads per unit of 2^(21 + Lw) configurations ----
-__global__ void __launch_bounds__(Z_THREADS)
+__global__ void __launch_bounds__(Z_THREADS, 3)
 zwalk_kernel(const Tables* __restrict__ tab, const ZTables* __restrict__ zt, Ctrl* __restrict__ ctrl,
              Entry* __restrict__ pool, unsigned* __restrict__ hist, const __grid_constant__ Plan plan)
 {
@@ -585,10 +585,17 @@ zwalk_kernel(const Tables* __restrict__ tab, const ZTables* __restrict__ zt, Ctr
             unsigned hits = __ballot_sync(0xffffffffu, !clear);
             flagged += __popc(hits);
             if (hits) {
-                // (out of line: the registers of this rare path must not weigh on the loop)
+                // (out of line: the registers of this rare path must not weigh on the loop; the arguments that go by
+                // reference are COPIES made here, so that Phi and tau themselves never have their address taken --
+                // otherwise they live in local memory and every step pays their stores)
+                int phi_copy[ZB];
+#pragma unroll
+                for (int i = 0; i < ZB; ++i) phi_copy[i] = Phi[i];
+                unsigned long long tau_copy = tau;
                 sub_true += handle_flagged(tab, ctrl, pool, hist, plan, reinterpret_cast<int*>(sA + (unsigned)warp * 8192u),
-                                           sDPhi + k * 16, sb, Phi, Eh, hits,
-                                           qW + ((unsigned long long)(t ^ (t >> 1)) << ZB), nlow, tau, lane);
+                                           sDPhi + k * 16, sb, phi_copy, Eh, hits,
+                                           qW + ((unsigned long long)(t ^ (t >> 1)) << ZB), nlow, tau_copy, lane);
+                tau = tau_copy;
                 tauE = tau_energy(tau);
             }
             // ---- move on to step t + 1 ----
