@@ -953,3 +953,30 @@ def test_tensor_core_accumulation_selftest(B):
         under, over = B.zscreen_selftest(seed)
         assert 0.0 <= under < 2.0 ** -14, under
         assert 0.0 <= over < 2.0 ** -14, over
+
+
+@pytest.mark.parametrize("seed", range(12))
+def test_tensor_core_screen_random_sweep(B, seed):
+    """Randomised differential test of the partition-function screen against the oracle: 25 spins, the screen forced on
+    (7/8 of the space goes through it unless the probe rejects it), instance family, field scale, sparsity and S drawn
+    per seed -- Gaussian, small integers with ties, mixed magnitudes, strong fields, diluted couplings. The screen can
+    only add work, so ANY instance must give the oracle's list; a wrong bound would show up as a missing state."""
+    rng = np.random.default_rng(7000 + seed)
+    N = 25
+    kind = seed % 4
+    if kind == 0:
+        J, h = I.complete_gaussian(N, seed=7100 + seed, h_scale=float(rng.choice([0.0, 0.3, 1.0, 3.0])))
+    elif kind == 1:
+        J, h = I.random_integer(N, seed=7200 + seed, wmax=int(rng.integers(1, 6)), density=float(rng.uniform(0.15, 1.0)))
+    elif kind == 2:
+        J, h = _wide_range_instance(N, 7300 + seed)
+    else:
+        U = rng.standard_normal((N, N)) * (rng.random((N, N)) < rng.uniform(0.2, 0.9))
+        J = np.triu(U, 1) + np.triu(U, 1).T
+        h = rng.standard_normal(N) * 10.0 ** rng.uniform(-1, 1.5)
+    S = int(rng.choice([1, 7, 100, 1000, 3000]))
+    q, e = _with_env({"ISING_Z_MIN_LOG2": 24}, lambda: gpu_lowest(B, J, h, S))
+    st = B.last_stats()
+    assert st.configs == 1 << N and st.kernel_variant in (16, 128)
+    qo, eo = oracle.lowest(J, h, S)
+    assert_exact(q, e, qo, eo)
