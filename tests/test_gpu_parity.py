@@ -980,3 +980,29 @@ def test_tensor_core_screen_random_sweep(B, seed):
     assert st.configs == 1 << N and st.kernel_variant in (16, 128)
     qo, eo = oracle.lowest(J, h, S)
     assert_exact(q, e, qo, eo)
+
+
+@pytest.mark.parametrize("kind", ["real", "int"])
+def test_qubo_and_zero_field_entry_points_through_the_tensor_core_screen(B, kind):
+    """qubo_lowest (mode 1 re-evaluation, widened band) and ising_lowest_h0 (half space + complements) with the
+    tensor-core screen forced on at 25 / 26 spins: the same expectations as their packed-kernel tests."""
+    N, S = 25, 500
+    a, b = _qubo_instance(N, 2500 + S, kind)
+    J = a / 4.0
+    h = b / 2.0 + a.sum(axis=1) / 4.0
+    q, e = _with_env({"ISING_Z_MIN_LOG2": 24}, lambda: B.qubo_lowest(a, b, S))
+    q = B.states_to_numpy(q); e = e.cpu().numpy()
+    assert B.last_stats().configs == 1 << N
+    qo, eo = oracle.lowest(J, h, S + 16)
+    assert e.tolist() == [_qubo_F(a, b, x) for x in q]
+    if kind == "int":
+        assert q.tolist() == qo[:S].tolist()
+    else:
+        W = np.abs(np.triu(J, 1)).sum() + np.abs(h).sum()
+        assert_real(q, e + (h.sum() - np.triu(J, 1).sum()), qo, eo, W, S, rel=1e-9)
+    # zero field, 26 spins: the enumerated half space has 2^25 states
+    J0, _ = (I.complete_gaussian(26, seed=2626) if kind == "real" else I.random_integer(26, seed=2627, wmax=2, density=0.6))
+    q2, e2 = _with_env({"ISING_Z_MIN_LOG2": 24}, lambda: B.ising_lowest_h0(J0, 200))
+    assert B.last_stats().configs == 1 << 25
+    qo2, eo2 = oracle.lowest(J0, np.zeros(26), 200)
+    assert_exact(B.states_to_numpy(q2), e2.cpu().numpy(), qo2, eo2)
