@@ -556,27 +556,34 @@ zwalk_kernel(const Tables* __restrict__ tab, const ZTables* __restrict__ zt, Ctr
                              : "r"(taddr) : "memory");
             }
             asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+            // Radix 4: two mid bits per stage, out = sum_{ab} x_ab (g_a g'_b) -- one multiply and three multiply-adds per
+            // output with four coefficient products formed once per step, instead of six operations in two radix-2
+            // stages: 84 packed operations per row instead of 126 (the coefficients are scalars broadcast to both lanes).
             unsigned long long part[4];
-            unsigned long long g0[7], g1[7];
+            unsigned long long cA[4], cB[4], cC[4];
 #pragma unroll
-            for (int i = 1; i < 7; ++i) { g0[i] = pk2(m0[i], m0[i]); g1[i] = pk2(m1[i], m1[i]); }
+            for (int ab = 0; ab < 4; ++ab) {
+                const float fa = ((ab & 1) ? m1[1] : m0[1]) * ((ab & 2) ? m1[2] : m0[2]);     // mid bits 1, 2 = spins 8, 9
+                const float fb = ((ab & 1) ? m1[3] : m0[3]) * ((ab & 2) ? m1[4] : m0[4]);     // mid bits 3, 4 = spins 10, 11
+                const float fc = ((ab & 1) ? m1[5] : m0[5]) * ((ab & 2) ? m1[6] : m0[6]);     // mid bits 5, 6 = spins 12, 13
+                cA[ab] = pk2(fa, fa); cB[ab] = pk2(fb, fb); cC[ab] = pk2(fc, fc);
+            }
 #pragma unroll
             for (int c = 0; c < 4; ++c) {
-                unsigned long long x[16];
+                // pair p covers mid = 32 c + 2p, 2p + 1; bit b of mid is bit b - 1 of p
+                unsigned long long y[4];
 #pragma unroll
-                for (int p = 0; p < 16; ++p) x[p] = pk2(__uint_as_float(v[c][2 * p]), __uint_as_float(v[c][2 * p + 1]));
-                // mid bits 1..4 = spins 8..11: pair p covers mid = 2p, 2p + 1; bit b of mid is bit b - 1 of p
+                for (int g = 0; g < 4; ++g) {
+                    unsigned long long x[4];
 #pragma unroll
-                for (int b = 1; b < 5; ++b) {
-#pragma unroll
-                    for (int p = 0; p < 16; p += (1 << b)) x[p] = fma2(x[p + (1 << (b - 1))], g1[b], mul2(x[p], g0[b]));
+                    for (int j = 0; j < 4; ++j)
+                        x[j] = pk2(__uint_as_float(v[c][2 * (4 * g + j)]), __uint_as_float(v[c][2 * (4 * g + j) + 1]));
+                    y[g] = fma2(x[3], cA[3], fma2(x[2], cA[2], fma2(x[1], cA[1], mul2(x[0], cA[0]))));
                 }
-                part[c] = x[0];
+                part[c] = fma2(y[3], cB[3], fma2(y[2], cB[2], fma2(y[1], cB[1], mul2(y[0], cB[0]))));
             }
-            // mid bits 5, 6 = spins 12, 13 (still in pairs), then mid bit 0 = spin 7 (inside the pair)
-            const unsigned long long h0 = fma2(part[1], g1[5], mul2(part[0], g0[5]));
-            const unsigned long long h1 = fma2(part[3], g1[5], mul2(part[2], g0[5]));
-            const unsigned long long hh = fma2(h1, g1[6], mul2(h0, g0[6]));
+            // mid bits 5, 6 select the chunk; mid bit 0 = spin 7 sits inside the pair and comes last
+            const unsigned long long hh = fma2(part[3], cC[3], fma2(part[2], cC[2], fma2(part[1], cC[1], mul2(part[0], cC[0]))));
             float Rlo, Rhi;
             upk2(hh, Rlo, Rhi);
             const float R = fmaf(Rhi, m1[0], Rlo * m0[0]);
