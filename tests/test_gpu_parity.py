@@ -1006,3 +1006,20 @@ def test_qubo_and_zero_field_entry_points_through_the_tensor_core_screen(B, kind
     assert B.last_stats().configs == 1 << 25
     qo2, eo2 = oracle.lowest(J0, np.zeros(26), 200)
     assert_exact(B.states_to_numpy(q2), e2.cpu().numpy(), qo2, eo2)
+
+
+def test_tensor_core_screen_with_the_largest_S(B):
+    """S = 65536 on 2^38 states: one block in 650 is flagged, the probe still accepts the screen (cost model in
+    csrc/api.cu), selection goes through the multi-block kernels. The packed kernel alone -- itself compared with the
+    oracle at S = 65536 on small instances (test_large_S) -- must return the same 65536 states and energies, and the
+    tier-3 oracle confirms the first 2000 of them."""
+    N, S = 38, 65536
+    J, h = I.complete_gaussian(N, seed=3838)
+    q, e = gpu_lowest(B, J, h, S)
+    assert B.last_stats().kernel_variant == 128
+    q2, e2 = _with_kernel(16, lambda: gpu_lowest(B, J, h, S))
+    assert B.last_stats().kernel_variant == 16
+    assert q.tolist() == q2.tolist() and e.tolist() == e2.tolist()
+    assert np.all(np.diff(e) >= 0) and len(set(q.tolist())) == S
+    qo, eo, _ = oracle.lowest_bnb(J, h, 2000, spare=16)
+    assert_exact(q[:2000], e[:2000], qo[:2000], eo[:2000])
