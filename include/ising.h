@@ -107,6 +107,31 @@ int ising_merge_lists(const uint64_t *states_in_dev, const double *energies_in_d
                       uint64_t *states_out_dev, double *energies_out_dev, void *stream);
 
 /*
+ * ising_merge_lists_static -- ising_merge_lists for callers that cannot allocate device memory. Same operation
+ * (PAPER.md:103-110), same arguments, same result bit for bit, for n <= ISING_MERGE_STATIC_MAX.
+ *
+ * Why it exists: every other compute entry point creates, on a host thread's first call, a workspace of about
+ * 130 MiB with cudaMalloc. A caller cannot do that when the device's memory already belongs, all of it, to another
+ * allocator in the same process (a framework that reserves the GPU at start-up), and does not want to when the
+ * device-wide synchronisation inside cudaMalloc / cudaFree would stall its other streams, or when the thread does
+ * nothing but merge the per-range lists of a sharded run. This entry point calls no cudaMalloc, cudaFree,
+ * cudaMallocHost or allocating library routine, ever: its sort scratch is a fixed 2 MiB array inside the library
+ * image (ISING_MERGE_STATIC_MAX entries of 16 bytes), resident on every GPU that loads the library until the process
+ * ends. Inputs and outputs remain the caller's buffers.
+ *
+ *   n > ISING_MERGE_STATIC_MAX          ISING_ERR_BAD_S, ising_last_error() names the limit; nothing is launched
+ *   first call on a device              also looks up the array's device address and sets a kernel attribute:
+ *                                       make it before any stream capture begins on that device
+ *   calls that overlap on the GPU       share the one array and RACE (wrong results, no error): serialise calls
+ *                                       per device. Back-to-back calls are fine: the array keeps the last call's
+ *                                       entries, but each call overwrites or pads every slot it later reads.
+ * Synchronises `stream` before returning, like ising_merge_lists.
+ */
+#define ISING_MERGE_STATIC_MAX 131072
+int ising_merge_lists_static(const uint64_t *states_in_dev, const double *energies_in_dev, int64_t n, int S,
+                             uint64_t *states_out_dev, double *energies_out_dev, void *stream);
+
+/*
  * ising_dos -- density of states (cf. the paper's Fig. 6): the histogram
  * of ALL 2^N energies of eq. (1). Every energy is formed exactly on the library's 2^-p grid (the instance rounded to
  * multiples of 2^-p; for integer / dyadic instances that is the instance itself, otherwise each energy is within

@@ -20,7 +20,7 @@ N_MAX = 63
 S_MAX = 65536
 
 # every symbol include/ising.h declares (tests/test_abi.py checks the header against this list and the .so)
-EXPORTS = ["ising_lowest", "ising_lowest_range", "ising_lowest_host", "ising_lowest_h0", "ising_lowest_alg1", "ising_dos", "ising_merge_lists", "qubo_lowest",
+EXPORTS = ["ising_lowest", "ising_lowest_range", "ising_lowest_host", "ising_lowest_h0", "ising_lowest_alg1", "ising_dos", "ising_merge_lists", "ising_merge_lists_static", "qubo_lowest",
            "ising_energies", "ising_get_last_stats", "ising_strerror", "ising_last_error", "ising_version",
            "ising_fma_peak", "ising_addmin_peak", "ising_addmin16x2_peak", "ising_addmin_mix_peak",
            "ising_zscreen_selftest", "ising_release_workspace"]
@@ -93,6 +93,8 @@ def load():
     lib.ising_lowest_range.argtypes = [dp, dp, i32, i32, u64, u64, up, dp, vp]
     lib.ising_lowest_host.argtypes = [dp, dp, i32, i32, u64, u64, up, dp, vp]
     lib.ising_merge_lists.argtypes = [up, dp, i64, i32, up, dp, vp]
+    lib.ising_merge_lists_static.argtypes = [up, dp, i64, i32, up, dp, vp]
+    lib.ising_merge_lists_static.restype = ctypes.c_int
     lib.ising_lowest_h0.argtypes = [dp, i32, i32, up, dp, vp]
     lib.ising_lowest_alg1.argtypes = [dp, dp, i32, i32, u64, u64, i32, up, dp, vp]
     lib.ising_lowest_alg1.restype = ctypes.c_int
@@ -289,6 +291,34 @@ def ising_merge_lists(states_in, energies_in, S: int, stream=None):
         rc = load().ising_merge_lists(states_in.data_ptr(), energies_in.data_ptr(), n, int(S),
                                       states.data_ptr(), energies.data_ptr(), _stream(stream))
     _check(rc, "ising_merge_lists")
+    return states, energies
+
+
+MERGE_STATIC_MAX = 131072
+
+
+def ising_merge_lists_static(states_in, energies_in, S: int, stream=None, out=None):
+    """`ising_merge_lists` without any device allocation inside the library (include/ising.h): for callers whose GPU
+    memory is already owned by another pool, or who cannot afford cudaMalloc's device-wide synchronisation. At most
+    MERGE_STATIC_MAX input pairs; the library's 2 MiB static scratch is shared, so do not overlap two calls on one
+    device. Pass `out=(states, energies)` (int64 [S], float64 [S] device tensors) and this wrapper allocates nothing
+    either; inputs must then already be contiguous int64 / float64."""
+    import torch
+    assert states_in.is_cuda and energies_in.is_cuda and states_in.dtype == torch.int64
+    states_in = states_in.contiguous()
+    energies_in = energies_in.to(torch.float64).contiguous()
+    n = states_in.numel()
+    if out is None:
+        states = torch.empty(S, dtype=torch.int64, device=states_in.device)
+        energies = torch.empty(S, dtype=torch.float64, device=states_in.device)
+    else:
+        states, energies = out
+        assert states.dtype == torch.int64 and energies.dtype == torch.float64
+        assert states.numel() >= S and energies.numel() >= S and states.is_contiguous() and energies.is_contiguous()
+    with torch.cuda.device(states_in.device):
+        rc = load().ising_merge_lists_static(states_in.data_ptr(), energies_in.data_ptr(), n, int(S),
+                                             states.data_ptr(), energies.data_ptr(), _stream(stream))
+    _check(rc, "ising_merge_lists_static")
     return states, energies
 
 

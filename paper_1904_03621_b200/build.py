@@ -12,7 +12,7 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
-SOURCES = ["api.cu", "stage.cu", "enumerate.cu", "enumerate16.cu", "zscreen.cu", "dos.cu", "select.cu", "peak.cu"]
+SOURCES = ["api.cu", "stage.cu", "enumerate.cu", "enumerate16.cu", "zscreen.cu", "dos.cu", "select.cu", "merge_static.cu", "peak.cu"]
 HEADERS = [os.path.join(CSRC, "common.cuh"), os.path.join(CSRC, "walk.cuh"), os.path.join(os.path.dirname(HERE), "include", "ising.h")]
 LIB = os.path.join(HERE, "libising_b200.so")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",

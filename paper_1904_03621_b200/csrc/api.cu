@@ -715,6 +715,9 @@ int check_args(const void* J, const void* h, int N, int S, unsigned long long q_
 }
 
 }  // namespace
+
+void set_last_error(const char* what) { t_last_error = what ? what : ""; }
+
 }  // namespace ising
 
 using namespace ising;

@@ -220,5 +220,7 @@ void launch_dos(const Tables* tab, int N, int Lw, unsigned long long base, unsig
 void launch_dos_direct(const Tables* tab, int N, int e_lo, int bshift, unsigned long long* hist, cudaStream_t st);
 // peak.cu
 double run_fma_peak(double ms_target, cudaStream_t st, int which);
+// api.cu: the calling thread's detail string behind ising_last_error(), for entry points that live in other files
+void set_last_error(const char* what);
 
 }  // namespace ising

@@ -65,6 +65,10 @@ def test_argument_validation_precedes_cuda(lib):
     assert lib.ising_lowest(Jp, hp, 99, 16, qp, ep, None) == B.ERR_BAD_N
     assert lib.ising_merge_lists(None, ep, 4, 2, qp, ep, None) == B.ERR_NULL
     assert lib.ising_merge_lists(qp, ep, 4, 5, qp, ep, None) == B.ERR_BAD_S
+    assert lib.ising_merge_lists_static(None, ep, 4, 2, qp, ep, None) == B.ERR_NULL
+    assert lib.ising_merge_lists_static(qp, ep, 4, 5, qp, ep, None) == B.ERR_BAD_S
+    assert lib.ising_merge_lists_static(qp, ep, B.MERGE_STATIC_MAX + 1, 2, qp, ep, None) == B.ERR_BAD_S   # beyond the static scratch
+    assert b"ISING_MERGE_STATIC_MAX" in lib.ising_last_error()
     assert lib.ising_energies(Jp, hp, 20, None, 4, ep, None) == B.ERR_NULL
     assert lib.ising_get_last_stats(None) == B.ERR_NULL
     assert lib.ising_lowest_h0(None, 20, 16, qp, ep, None) == B.ERR_NULL
