@@ -20,7 +20,8 @@
  * block that passes a screen is formed exactly in 32-bit integers; both screens can only add work
  * (false hits), never lose a state (DESIGN.md sections 6, 6b). Environment knobs (development /
  * tests): ISING_KERNEL = 16 (packed screen only) | 32 (int32 add-min per configuration, no screen),
- * ISING_Z_MIN_LOG2, ISING_Z_RAMP_LOG2, ISING_LW, ISING_CHUNK_LOG2, ISING_GROWTH, ISING_PATH = 1
+ * ISING_Z_MIN_LOG2, ISING_Z_RAMP_LOG2, ISING_Z_FORCE = 1 (the bulk takes the tensor-core screen whatever its probe
+ * flagged), ISING_LW, ISING_CHUNK_LOG2, ISING_GROWTH, ISING_PATH = 1
  * (host-sequenced pieces), ISING_KEEP_CAP_LOG2.
  *
  * Pointer arguments say in their name where they live: *_dev = device memory, *_host = host memory.
@@ -224,32 +225,33 @@ const char *ising_strerror(int status);
 const char *ising_last_error(void);   /* thread-local detail string of the last failure */
 int ising_version(void);
 
-/* FP32-FMA microbenchmark (the roofline denominator): runs a dependency-free FFMA kernel for roughly
- * `ms_target` milliseconds on `stream` and writes the measured FMA/s (lane-FMAs per second, whole GPU). */
+/* FP32-FMA microbenchmark (denominator of BASELINE.json's "FP32 FMA roofline" yardstick, bench.py `fp32_fma_roofline`):
+ * runs a dependency-free FFMA kernel for roughly `ms_target` milliseconds on `stream` and writes the measured FMA/s
+ * (lane-FMAs per second, whole GPU). */
 int ising_fma_peak(double ms_target, double *fma_per_s_out_host, void *stream);
 
 /* Same for the enumeration's inner operation, one fused integer add-min (SASS VIADDMNMX) per configuration:
- * lane add-mins per second, whole GPU. This is the ALU ceiling the `roofline` of bench.py is quoted against
- * (DESIGN.md "Roofline"). */
+ * lane add-mins per second, whole GPU. This is the ALU ceiling bench.py's `roofline_int32` (the int32 kernel, ISING_KERNEL=32) is
+ * quoted against; the default path's `roofline` is a tensor-core roofline. */
 int ising_addmin_peak(double ms_target, double *addmin_per_s_out_host, void *stream);
 
-/* Same for the packed inner operation of the default kernel (SASS VIADDMNMX.U16x2): lane INSTRUCTIONS per second,
+/* Same for the packed inner operation of the packed-screen kernel (SASS VIADDMNMX.U16x2): lane INSTRUCTIONS per second,
  * whole GPU; each instruction forms two 16-bit add-mins, i.e. screens two configurations, so the configuration
  * ceiling of the packed kernel is twice this number. */
 int ising_addmin16x2_peak(double ms_target, double *inst_per_s_out_host, void *stream);
 
-/* The instruction MIX the default kernel is built from, register-only: per chain step one fused VIADDMNMX.U16x2
+/* The instruction MIX the packed-screen kernel (walk_kernel<Inner16>) is built from, register-only: per chain step one fused VIADDMNMX.U16x2
  * (two 16-bit add-mins, ALU pipe) and one split group IMAD + IMAD + VIMNMX3.U16x2 (four add-mins: two packed sums on
  * the FMA pipe, one three-way packed minimum on the ALU pipe). Writes lane ADD-MINS per second, whole GPU: the
  * measured counterpart of the derived bound of DESIGN.md 5.2 (192 add-mins per clock per SM) and the denominator of
- * bench.py's `roofline.peak`. */
+ * bench.py's `roofline_packed16.peak`. */
 int ising_addmin_mix_peak(double ms_target, double *addmin_per_s_out_host, void *stream);
 
 /* Self-test of the hardware property the tensor-core screen's proof relies on (csrc/zscreen.cu): one
  * 128 x 128 x 128 bf16 tcgen05 GEMM of pseudo-random POSITIVE operands spanning 2^-100 .. 2^40, fp32 accumulation in
  * tensor memory, compared entry by entry with the same sums formed in fp64 from the same bf16 values. Writes the
- * largest relative UNDER-estimate (ref - D) / ref and over-estimate (D - ref) / ref. The screen's margin (0.03 bits,
- * i.e. 2.1 %) budgets 2^-14 for this term. */
+ * largest relative UNDER-estimate (ref - D) / ref and over-estimate (D - ref) / ref. The screen's margin (0.05 bits,
+ * i.e. 3.5 %) budgets 2^-14 for this term. */
 int ising_zscreen_selftest(uint32_t seed, double *rel_under_out_host, double *rel_over_out_host, void *stream);
 
 /* Frees the calling thread's cached workspace (device pool, tables, pinned control block). Optional. */

@@ -160,7 +160,7 @@ struct Run {
     Workspace* ws;
     ising_stats* stats;
     const double *J, *h, *Jorig, *horig;
-    int mode, N, S, variant, lw_max, chunk_log2, growth, qshift, z_min_log2, z_ramp_log2;
+    int mode, N, S, variant, lw_max, chunk_log2, growth, qshift, z_min_log2, z_ramp_log2, z_force;
     unsigned keep_cap;
     unsigned long long q_begin, q_end;
     cudaStream_t st;
@@ -206,6 +206,20 @@ int launch_walk(const Run& r, const Plan& plan)
     LAUNCH_CHECK(r.variant != 32 ? "walk_kernel<Inner16>" : "walk_kernel<Inner32>");
     r.stats->kernel_launches += 1;
     r.stats->enum_launches += 1;
+    return ISING_OK;
+}
+
+// One launch of the tensor-core screen. The grid is one CTA per unit: a count that does not fit the grid's x extent
+// (N near 63 in one call, or a small ISING_LW on a huge range) is refused here instead of being truncated.
+int launch_z(const Run& r, const Plan& plan)
+{
+    Workspace& ws = *r.ws;
+    if (plan.total_units == 0 || plan.total_units > 0x7fffffffull) {
+        t_last_error = "internal: unit count of the tensor-core screen does not fit one launch (split the range)";
+        return ISING_ERR_INTERNAL;
+    }
+    launch_zwalk(ws.tab, ws.zt, ws.ctrl, ws.pool, ws.hist, plan, r.st);
+    LAUNCH_CHECK("zwalk_kernel");
     return ISING_OK;
 }
 
@@ -304,8 +318,13 @@ int run_single_pass(Run& r, unsigned long long* states_out, double* energies_out
     plan_header(r, plan, 1, INT32_MIN);
     const unsigned long long range = r.q_end - r.q_begin;
     const bool direct = r.N <= N_DIRECT_MAX;
+    // The screen's units are 2^21 states, aligned; range bounds are multiples of 2^20 only (include/ising.h). A ragged
+    // head (q_begin an odd multiple of 2^20) is absorbed by the packed ramp-up, which then ends at the next multiple
+    // of 2^21; a ragged tail [z_end, q_end) of 2^20 states follows the bulk launch through the packed kernel.
+    const unsigned long long zmask = (1ull << (ZB + 7)) - 1ull;
     const bool use_z = !direct && (r.variant == 0 || r.variant == 128) && range >= (1ull << r.z_min_log2) &&
-                       range >= (1ull << (ZB + 7 + 3)) && (r.q_begin & ((1ull << (ZB + 7)) - 1ull)) == 0;
+                       range >= (1ull << (ZB + 7 + 3));
+    const unsigned long long z_end = r.q_end & ~zmask;                    // end of the screen's stretch
     int rc = ISING_OK;
     auto timed_launch = [&](auto&& launch) -> int {
         CUDA_TRY(cudaEventRecord(ws.ev[2], r.st));
@@ -342,7 +361,10 @@ int run_single_pass(Run& r, unsigned long long* states_out, double* energies_out
         while (X > prime && X * (unsigned long long)r.S > (1ull << 35)) X >>= 1;
         if (X > range) X = range;
         unsigned long long p0 = range;                                   // end of the packed kernel's stretch
-        if (use_z) { p0 = 1ull << r.z_ramp_log2; while (p0 > range / 8) p0 >>= 1; }
+        if (use_z) { p0 = 1ull << r.z_ramp_log2; while (p0 > range / 8) p0 >>= 1; }       // 2^21 <= p0 <= range / 8
+        // states [q_begin, ramp_end) go through the packed kernel, [ramp_end, probe_end) are the probe of the screen
+        const unsigned long long ramp_end = use_z ? (r.q_begin + p0 + zmask) & ~zmask : r.q_end;
+        const unsigned long long probe_end = ramp_end + p0;               // <= z_end because range >= 8 p0 >= 2^24
         int ns = 0;
         unsigned long long cur = r.q_begin, units = 0;
         plan.seg[ns++] = Segment{cur, units, prime >> LOWBITS, 0ull, LOWBITS, 0};
@@ -351,7 +373,7 @@ int run_single_pass(Run& r, unsigned long long* states_out, double* energies_out
             plan.seg[ns++] = Segment{cur, units, (X - prime) >> LOWBITS, prime, LOWBITS, 0};
             units += (X - prime) >> LOWBITS; cur += X - prime;
         }
-        rc = plan_walk_segments(r, plan, ns, cur, units, r.q_begin + p0, prime);
+        rc = plan_walk_segments(r, plan, ns, cur, units, ramp_end, prime);
         if (rc != ISING_OK) return rc;
         plan.nseg = ns;
         plan.total_units = units;
@@ -365,7 +387,7 @@ int run_single_pass(Run& r, unsigned long long* states_out, double* energies_out
             Plan zp;
             plan_header(r, zp, 1, INT32_MIN);
             ns = 0; units = 0;
-            rc = plan_z_segments(r, zp, ns, cur, units, r.q_begin + 2 * p0, false);
+            rc = plan_z_segments(r, zp, ns, cur, units, probe_end, false);
             if (rc != ISING_OK) return rc;
             zp.nseg = ns; zp.total_units = units;
             CUDA_TRY(cudaEventRecord(ws.ev[3], r.st));                   // (the ramp-up launch ends here)
@@ -373,33 +395,43 @@ int run_single_pass(Run& r, unsigned long long* states_out, double* energies_out
             if (rc != ISING_OK) return rc;
             if ((rc = add_elapsed()) != ISING_OK) return rc;
             if (ws.h_ctrl->status != ISING_OK) return ISING_OK;
-            rc = timed_launch([&]() -> int {
-                launch_zwalk(ws.tab, ws.zt, ws.ctrl, ws.pool, ws.hist, zp, r.st);
-                LAUNCH_CHECK("zwalk_kernel");
-                return ISING_OK;
-            });
+            rc = timed_launch([&]() -> int { return launch_z(r, zp); });
             if (rc != ISING_OK) return rc;
             r.stats->kernel_launches += 3;
             r.stats->enum_launches += 1;
             r.stats->z_launches += 1;
             last_was_z = true;
-            last_z_configs = p0;
+            last_z_configs = probe_end - ramp_end;
             rc = read_ctrl(r);
             if (rc != ISING_OK) return rc;
             if ((rc = add_elapsed()) != ISING_OK) return rc;
             const double zs = (double)ws.h_ctrl->z_steps, zf = (double)ws.h_ctrl->z_flagged;
-            // A flagged block costs its CTA about 20 us, a clean step (128 blocks) 1.8 us, and the packed kernel is 14 times
-            // slower than the clean screen: the screen wins up to about 1 flagged block in 27. The probe sees the loosest
-            // threshold of the bulk, so its rate is an upper bound.
-            const bool z_ok = !ws.h_ctrl->pool_overflow && zs > 0.0 && zf * 48.0 <= zs;
+            // Cost model behind the constant 48: a clean step (128 blocks, one per thread) takes 1.8 us and the packed
+            // kernel is 14 times slower, i.e. 25 us for the same 2^21 states; a flagged block takes its WARP about 20 us.
+            // If the flagged blocks of a step spread evenly over the CTA's four warps the screen breaks even at about
+            // 1 flagged block in 27, if they all fall to one warp at 1 in 109. 1 in 48 sits between the two and is
+            // the rate up to which the screen was measured to win (N = 42, S = 65536: 22 ms against 135 ms). The probe
+            // runs under the loosest threshold of the bulk, but it is only a sample: an instance whose low states cluster
+            // late in q order can flag more often later on. That costs time, never a state.
+            // ISING_Z_FORCE = 1 (tests): the bulk takes the screen whatever the probe flagged, so that the flagged-block
+            // path is compared with the oracle under load.
+            const bool z_ok = !ws.h_ctrl->pool_overflow && zs > 0.0 && (r.z_force || zf * 48.0 <= zs);
             reset_queue_kernel<<<1, 1, 0, r.st>>>(ws.ctrl, 0);
             r.stats->kernel_launches += 1;
             Plan rest;
             plan_header(r, rest, 1, INT32_MIN);
             ns = 0; units = 0;
+            Plan tail;                                                   // z_ok and a ragged end: [z_end, q_end), packed kernel
+            plan_header(r, tail, 1, INT32_MIN);
             if (z_ok) {
-                rc = plan_z_segments(r, rest, ns, cur, units, r.q_end, true);
+                rc = plan_z_segments(r, rest, ns, cur, units, z_end, true);
                 r.stats->kernel_variant = 128;
+                if (rc == ISING_OK && z_end < r.q_end) {
+                    tail.seg[0] = Segment{z_end, 0ull, (r.q_end - z_end) >> MIN_CHUNK_BITS, 0ull, MIN_CHUNK_BITS, 0};
+                    tail.nseg = 1;
+                    tail.total_units = tail.seg[0].n_units;
+                    cur = r.q_end;
+                }
             } else {
                 rc = plan_walk_segments(r, rest, ns, cur, units, r.q_end, 0ull);
             }
@@ -408,15 +440,20 @@ int run_single_pass(Run& r, unsigned long long* states_out, double* energies_out
             if (cur != r.q_end) { t_last_error = "internal: work plan does not cover the range"; return ISING_ERR_INTERNAL; }
             rc = timed_launch([&]() -> int {
                 if (!z_ok) return launch_walk(r, rest);
-                launch_zwalk(ws.tab, ws.zt, ws.ctrl, ws.pool, ws.hist, rest, r.st);
-                LAUNCH_CHECK("zwalk_kernel");
+                const int zrc = launch_z(r, rest);
+                if (zrc != ISING_OK) return zrc;
                 r.stats->kernel_launches += 1;
                 r.stats->enum_launches += 1;
                 r.stats->z_launches += 1;
+                if (tail.nseg) {
+                    reset_queue_kernel<<<1, 1, 0, r.st>>>(ws.ctrl, 0);
+                    r.stats->kernel_launches += 1;
+                    return launch_walk(r, tail);
+                }
                 return ISING_OK;
             });
             if (rc != ISING_OK) return rc;
-            if (z_ok) { last_was_z = true; last_z_configs = r.q_end - (r.q_begin + 2 * p0); }
+            if (z_ok) { last_was_z = true; last_z_configs = z_end - probe_end; }
         } else if (cur != r.q_end) {
             t_last_error = "internal: work plan does not cover the range";
             return ISING_ERR_INTERNAL;
@@ -588,6 +625,7 @@ int run_lowest(const double* J, const double* h, const double* Jorig, const doub
     r.variant = kv == 32 ? 32 : (kv == 16 ? 16 : 0);
     r.z_min_log2 = env_int("ISING_Z_MIN_LOG2", 36, ZB + 10, 63);
     r.z_ramp_log2 = env_int("ISING_Z_RAMP_LOG2", 34, ZB + 7, 44);
+    r.z_force = env_int("ISING_Z_FORCE", 0, 0, 1);
     // test knob for the band pass: a selection keeps at most 2^k entries (never fewer than S)
     r.keep_cap = 1u << env_int("ISING_KEEP_CAP_LOG2", 20, 5, 20);
     while (r.keep_cap < (unsigned)S) r.keep_cap <<= 1;

@@ -802,12 +802,14 @@ def test_sharded_exchange_path_over_nccl_single_rank(B):
 
 
 # ---------- the multi-rank path with the REAL C-ABI calls: two processes share the one GPU, gloo for the exchange ----------
-def _sharded_gpu_worker(rank, world, port, out_dir):
+def _sharded_gpu_worker(rank, world, port, out_dir, z_min_log2=0):
     import torch
     import torch.distributed as dist
     from paper_1904_03621_b200 import binding as Bw, sharded
     os.environ["MASTER_ADDR"] = "127.0.0.1"
     os.environ["MASTER_PORT"] = str(port)
+    if z_min_log2:
+        os.environ["ISING_Z_MIN_LOG2"] = str(z_min_log2)        # per-rank ranges of 2^34..2^35 states take the tensor-core screen
     torch.cuda.set_device(0)
     dist.init_process_group("gloo", rank=rank, world_size=world)
     try:
@@ -817,25 +819,33 @@ def _sharded_gpu_worker(rank, world, port, out_dir):
         np.save(os.path.join(out_dir, f"q{rank}.npy"), Bw.states_to_numpy(q))
         np.save(os.path.join(out_dir, f"e{rank}.npy"), e.cpu().numpy())
         st = Bw.last_stats()
-        np.save(os.path.join(out_dir, f"n{rank}.npy"), np.array([st.kernel_launches]))
+        np.save(os.path.join(out_dir, f"n{rank}.npy"), np.array([st.kernel_launches, st.kernel_variant, st.z_blocks, st.configs]))
     finally:
         dist.destroy_process_group()
 
 
-@pytest.mark.parametrize("world", [2, 3])
-def test_sharded_two_processes_on_one_gpu(B, golden_dir, tmp_path, world):
+@pytest.mark.parametrize("world,z_min_log2", [(2, 0), (3, 0), (2, 30), (3, 30)])
+def test_sharded_two_processes_on_one_gpu(B, golden_dir, tmp_path, world, z_min_log2):
     """SURVEY.md 8(e) end to end: every rank enumerates its own range of cfg3 with the real kernels, the lists are
     exchanged with one all-gather (gloo: NCCL refuses several ranks on one device) and merged by ising_merge_lists
-    on every rank. Every rank must end with the stored oracle list."""
+    on every rank. Every rank must end with the stored oracle list. With z_min_log2 = 30 every rank's range (2^35
+    states, or a third of 2^36 with bounds at odd multiples of 2^20) goes through the tensor-core screen, as every
+    rank's 2^45 states would at N = 48 on 8 GPUs."""
     import socket
     import torch.multiprocessing as mp
     s = socket.socket(); s.bind(("127.0.0.1", 0)); port = s.getsockname()[1]; s.close()
-    mp.spawn(_sharded_gpu_worker, args=(world, port, str(tmp_path)), nprocs=world, join=True)
+    mp.spawn(_sharded_gpu_worker, args=(world, port, str(tmp_path), z_min_log2), nprocs=world, join=True)
     c = I.baseline_config(3)
     qo, eo = load_golden(os.path.join(golden_dir, "cfg3.txt"))
+    total = 0
     for r in range(world):
         q = np.load(tmp_path / f"q{r}.npy"); e = np.load(tmp_path / f"e{r}.npy")
         assert_exact(q, e, qo[:c.S], eo[:c.S])
+        _, variant, z_blocks, configs = np.load(tmp_path / f"n{r}.npy").tolist()
+        total += configs
+        if z_min_log2:
+            assert variant == 128 and z_blocks > 0, (r, variant, z_blocks)
+    assert total == 1 << c.N
 
 
 _FIRST_CALL_SCRIPT = r"""
@@ -924,11 +934,18 @@ def test_tensor_core_screen_small(B, name):
         J, h = np.zeros((24, 24)), np.zeros(24); S = 40
     q, e = _with_env({"ISING_Z_MIN_LOG2": 24}, lambda: gpu_lowest(B, J, h, S))
     st = B.last_stats()
-    assert st.configs == 1 << len(h) and st.kernel_variant in (16, 128)
+    # (all-zero couplings: every state ties, the single pass overflows the pool and the piecewise redo never screens)
+    assert st.configs == 1 << len(h) and st.kernel_variant in (16, 128) and (st.z_blocks > 0 or st.passes > 1)
     if name == "mattis30":
         qo, eo = oracle.lowest_gray(J, h, S)
     else:
         qo, eo = oracle.lowest(J, h, S)
+    assert_exact(q, e, qo, eo)
+    # again with the probe's verdict overruled: the BULK goes through zwalk_kernel whatever the flag rate, so the
+    # flagged-block path (handle_flagged / form_flagged / push_block of zscreen.cu) is compared with the oracle under load
+    q, e = _with_env({"ISING_Z_MIN_LOG2": 24, "ISING_Z_FORCE": 1}, lambda: gpu_lowest(B, J, h, S))
+    st2 = B.last_stats()
+    assert st2.passes > 1 or (st2.kernel_variant == 128 and st2.z_launches == 2 and st2.z_blocks > st.z_blocks * (st.kernel_variant != 128))
     assert_exact(q, e, qo, eo)
 
 
@@ -977,8 +994,12 @@ def test_tensor_core_screen_random_sweep(B, seed):
     S = int(rng.choice([1, 7, 100, 1000, 3000]))
     q, e = _with_env({"ISING_Z_MIN_LOG2": 24}, lambda: gpu_lowest(B, J, h, S))
     st = B.last_stats()
-    assert st.configs == 1 << N and st.kernel_variant in (16, 128)
+    assert st.configs == 1 << N and st.kernel_variant in (16, 128) and (st.z_blocks > 0 or st.passes > 1)
     qo, eo = oracle.lowest(J, h, S)
+    assert_exact(q, e, qo, eo)
+    q, e = _with_env({"ISING_Z_MIN_LOG2": 24, "ISING_Z_FORCE": 1}, lambda: gpu_lowest(B, J, h, S))     # bulk forced through the screen
+    st2 = B.last_stats()
+    assert st2.passes > 1 or (st2.kernel_variant == 128 and st2.z_launches == 2)
     assert_exact(q, e, qo, eo)
 
 
@@ -1023,3 +1044,39 @@ def test_tensor_core_screen_with_the_largest_S(B):
     assert np.all(np.diff(e) >= 0) and len(set(q.tolist())) == S
     qo, eo, _ = oracle.lowest_bnb(J, h, 2000, spare=16)
     assert_exact(q[:2000], e[:2000], qo[:2000], eo[:2000])
+
+
+@pytest.mark.parametrize("k,m", [(1, 127), (3, 64), (0, 77), (5, 128), (33, 57)])
+def test_tensor_core_screen_on_ranges_ragged_at_2_pow_20(B, k, m):
+    """Range bounds are multiples of 2^20 (include/ising.h) but the screen's units are 2^21 states: a range that begins
+    or ends at an ODD multiple of 2^20 gets its ragged head from the packed ramp-up and its ragged tail from one extra
+    packed launch (csrc/api.cu, run_single_pass). 27 spins, the screen forced on; the list of every such range must
+    be the oracle's list of the same range, and the screen must really have run."""
+    J, h = I.complete_gaussian(27, seed=2727)
+    lo, hi = k << 20, m << 20
+    S = 100
+    q, e = _with_env({"ISING_Z_MIN_LOG2": 24, "ISING_Z_FORCE": 1}, lambda: gpu_lowest(B, J, h, S, lo, hi))
+    st = B.last_stats()
+    assert st.configs == hi - lo and st.z_blocks > 0 and st.kernel_variant == 128 and st.z_launches == 2
+    qo, eo = oracle.lowest(J, h, S, lo, hi)
+    assert_exact(q, e, qo, eo)
+
+
+def test_three_way_shard_ranges_through_the_tensor_core_screen(B):
+    """sharded.shard_ranges(N, 3) cuts 2^N into ranges whose inner bounds are odd multiples of 2^20 (2^N / 2^20 is not
+    divisible by 3). Each of the three ranges through the real solver with the screen forced on, then the merge: the
+    oracle's list of the whole space. (A world of three is what `bench.py --gpus 3` or any non-power-of-two job makes.)"""
+    import torch
+    from paper_1904_03621_b200 import sharded
+    J, h = I.random_integer(27, seed=2733, wmax=3, density=0.6)
+    S = 300
+    ranges = sharded.shard_ranges(27, 3)
+    assert any((lo >> 20) & 1 or (hi >> 20) & 1 for lo, hi in ranges)
+    parts = []
+    for lo, hi in ranges:
+        parts.append(_with_env({"ISING_Z_MIN_LOG2": 24, "ISING_Z_FORCE": 1}, lambda: B.ising_lowest_range(J, h, S, lo, hi)))
+        st = B.last_stats()
+        assert st.configs == hi - lo and st.z_blocks > 0 and st.kernel_variant == 128
+    qm, em = B.ising_merge_lists(torch.cat([p[0] for p in parts]), torch.cat([p[1] for p in parts]), S)
+    qo, eo = oracle.lowest(J, h, S)
+    assert_exact(B.states_to_numpy(qm), em.cpu().numpy(), qo, eo)
