@@ -38,14 +38,17 @@ if ROOT not in sys.path:
 
 METRIC = "spin_configs_evaluated_per_s"
 UNIT = "configs/s"
-# integer-ALU ceiling of the inner operation: VIADDMNMX issues on the ALU pipe at
-# 148 SMs x 4 sub-partitions x 16 lanes/clk (B300_MICROARCH.md "Pipe rates") x 1.965 GHz (MEASURED_PEAKS.json);
-# the default kernel's VIADDMNMX.U16x2 forms two 16-bit add-mins (two configurations) per lane instruction,
-# the int32 kernel (ISING_KERNEL=32) one. The default kernel also forms part of its sums as packed adds on the FMA
-# pipe and takes the minimum of two of them with one VIMNMX3.U16x2 (4 configurations per ALU lane instruction, 3 issue
-# slots); with the ALU pipe at 16 lanes/clk and one warp instruction issued per clock per sub-partition the best
-# possible mix of the two forms is 48 configurations/clk/sub-partition = 192 per SM: that bound is
-# `roofline.peak`; the ceiling of the fused form alone (128 per SM) is reported beside it.
+# `roofline` (the default path's dominant kernel, zwalk_kernel) is a TENSOR roofline against MEASURED_PEAKS.json.
+# The constants below serve the two ALU kernels' own objects, `roofline_packed16` and `roofline_int32` (DESIGN.md
+# "Roofline"): VIADDMNMX issues on the ALU pipe at 148 SMs x 4 sub-partitions x 16 lanes/clk (B300_MICROARCH.md "Pipe
+# rates") x 1.965 GHz (MEASURED_PEAKS.json); the packed kernel's VIADDMNMX.U16x2 (ISING_KERNEL=16; it also ramps the
+# threshold up for the default path) forms two 16-bit add-mins (two configurations) per lane instruction, the int32
+# kernel (ISING_KERNEL=32) one. The packed kernel also forms part of its sums as packed adds on the FMA pipe and takes
+# the minimum of two of them with one VIMNMX3.U16x2 (4 configurations per ALU lane instruction, 3 issue slots); with
+# the ALU pipe at 16 lanes/clk and one warp instruction issued per clock per sub-partition the best possible mix of the
+# two forms is 48 configurations/clk/sub-partition = 192 per SM. The `peak` of both ALU objects is the
+# MEASURED rate of the kernel's own instruction mix (microbenchmarks run in this invocation); the derived bounds are
+# reported beside it.
 ALU_LANES_PER_CLK_PER_SM = 64
 MIX_BOUND_CONFIGS_PER_CLK_PER_SM = 192
 FMA_LANES_PER_CLK_PER_SM = 128
@@ -429,6 +432,10 @@ def main():
                                 "operand row and folds its accumulator row on the CUDA cores (DESIGN.md 5.1c), and the "
                                 "first 2^35 states go through the packed ALU kernel (roofline_packed16)"}
             dtype = "bf16 tensor-core screen (fp32 accumulate) + int16x2 screen + int32 exact (fp64 output)"
+            evaluated = ("bf16 partition-function term per configuration (tensor-core screen of 2^14-configuration blocks); "
+                         "exact int32 energy for every configuration of a flagged block and of the packed ramp-up's hit "
+                         "blocks; `value` counts configurations SCREENED, `value_int32` configurations whose int32 energy "
+                         "is formed one by one (ISING_KERNEL=32)")
         else:
             roofline = alu_roofline(st.kernel_variant, enum_rate, enum_launches, enum_ms)
             traffic = profile_number("enumerate_dram_bytes_per_launch.txt")
@@ -437,11 +444,15 @@ def main():
                                           "profiles/enumerate_dram_bytes_per_launch.txt; not re-measured in this run"
                                           if traffic is not None else None)
             dtype = "int16x2 screen + int32 exact (fp64 output)" if st.kernel_variant == 16 else "int32 (fp64 output)"
+            evaluated = ("16-bit lower bound per configuration (packed screen); exact int32 energy for every configuration of "
+                         "a hit block" if st.kernel_variant == 16 else "exact int32 energy per configuration")
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": dev_ms_max / args.steps, "higher_is_better": True,
             "scaling": "strong" if (sharded_mode and world > 1) else "weak", "vs_baseline": None,
             "dtype": dtype,
+            "evaluated": evaluated,
+            "value_int32": None,        # filled below from the int32 pass of this invocation (the strict-reading figure)
             "data": "synthetic",
             "config": {"workload": f"BASELINE.json configs[{args.config - 1}]: {inst.name}, N={N}, S={S}, "
                                    f"states [0, 2^{q_end.bit_length() - 1}) of 2^{N} per step",
@@ -476,6 +487,8 @@ def main():
                             "steps": rr["steps"], "same_list_as_default_path": True,
                             "dtype": "int16x2 screen + int32 exact (fp64 output)" if kv == 16 else "int32 (fp64 output)"})
                 line[key] = obj
+                if kv == 32:
+                    line["value_int32"] = obj["configs_per_s"]
         if e2e:
             line["e2e"] = {"value": total_configs / e2e_s_max, "unit": UNIT,
                            "h2d_bytes_per_step": e2e["h2d"], "d2h_bytes_per_step": e2e["d2h"]}
