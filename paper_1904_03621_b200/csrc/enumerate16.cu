@@ -114,13 +114,12 @@ struct Inner16 {
     // a3: 1024 configurations, one packed add-min per two of them; a4: the screen on the lower bound,
     //   bound * 2^s + Eh <= tauE  <=>  bound <= (tauE - Eh) >> s
     // Which of the chunks 1..7 of a row use the split form (bit x of E16_P1MASK), and the statement order of the two
-    // register sets inside a fused chunk (E16_ORDER), decide how ptxas schedules the loop. Measured on B200, 2^43-state
-    // slice of cfg5, configurations/s (all variants have 0 register-bank conflicts):
+    // register sets inside a fused chunk, decide how ptxas schedules the loop. Measured on B200, 2^43-state slice of
+    // cfg5, configurations/s (all variants have 0 register-bank conflicts; order 0 = a then b per word of C, the default
+    // of the mask sweep; order 1 = b then a per word, the one kept below; order 2 = all of a, then all of b; two mixed
+    // orders, a first where C sits in an even register and the reverse, were no better and are not listed):
     //   mask 0xC0: 3.34e13   0x06: 3.39e13   0x82: 3.36e13   0x60: 3.25e13   0x80: 3.27e13   0xE0: 3.42e13   0x46: 3.40e13
-    //   0x1E: 3.37e13   0xF0: 3.29e13   0xAA: 3.30e13   0xE0 + order 1: 3.45e13 (default)   0xE0 + order 2: 3.41e13
-#ifndef E16_ORDER
-#define E16_ORDER 1
-#endif
+    //   0x1E: 3.37e13   0xF0: 3.29e13   0xAA: 3.30e13   0xE0 + order 1: 3.45e13 (kept)   0xE0 + order 2: 3.41e13
 #ifndef E16_P1MASK
 #define E16_P1MASK 0xE0          // chunks 5, 6 and 7 of every row in the split form
 #endif
@@ -163,52 +162,16 @@ struct Inner16 {
                     mb = __vimin3_u16x2(mb, b0, b1);
                     ma = __vimin3_u16x2(ma, a2, a3);
                     mb = __vimin3_u16x2(mb, b2, b3);
-                } else if (E16_ORDER == 0) {
-                    ma = __viaddmin_u16x2(R.Va[4 * x + 0], c.x, ma);
-                    mb = __viaddmin_u16x2(R.Vb[4 * x + 0], c.x, mb);
-                    ma = __viaddmin_u16x2(R.Va[4 * x + 1], c.y, ma);
-                    mb = __viaddmin_u16x2(R.Vb[4 * x + 1], c.y, mb);
-                    ma = __viaddmin_u16x2(R.Va[4 * x + 2], c.z, ma);
-                    mb = __viaddmin_u16x2(R.Vb[4 * x + 2], c.z, mb);
-                    ma = __viaddmin_u16x2(R.Va[4 * x + 3], c.w, ma);
-                    mb = __viaddmin_u16x2(R.Vb[4 * x + 3], c.w, mb);
-                } else if (E16_ORDER == 3) {
-                    // a first where C sits in an even register, b first where it sits in an odd one (see file header)
-                    ma = __viaddmin_u16x2(R.Va[4 * x + 0], c.x, ma);
-                    mb = __viaddmin_u16x2(R.Vb[4 * x + 0], c.x, mb);
-                    mb = __viaddmin_u16x2(R.Vb[4 * x + 1], c.y, mb);
-                    ma = __viaddmin_u16x2(R.Va[4 * x + 1], c.y, ma);
-                    ma = __viaddmin_u16x2(R.Va[4 * x + 2], c.z, ma);
-                    mb = __viaddmin_u16x2(R.Vb[4 * x + 2], c.z, mb);
-                    mb = __viaddmin_u16x2(R.Vb[4 * x + 3], c.w, mb);
-                    ma = __viaddmin_u16x2(R.Va[4 * x + 3], c.w, ma);
-                } else if (E16_ORDER == 4) {
-                    mb = __viaddmin_u16x2(R.Vb[4 * x + 0], c.x, mb);
-                    ma = __viaddmin_u16x2(R.Va[4 * x + 0], c.x, ma);
-                    ma = __viaddmin_u16x2(R.Va[4 * x + 1], c.y, ma);
-                    mb = __viaddmin_u16x2(R.Vb[4 * x + 1], c.y, mb);
-                    mb = __viaddmin_u16x2(R.Vb[4 * x + 2], c.z, mb);
-                    ma = __viaddmin_u16x2(R.Va[4 * x + 2], c.z, ma);
-                    ma = __viaddmin_u16x2(R.Va[4 * x + 3], c.w, ma);
-                    mb = __viaddmin_u16x2(R.Vb[4 * x + 3], c.w, mb);
-                } else if (E16_ORDER == 1) {
-                    mb = __viaddmin_u16x2(R.Vb[4 * x + 0], c.x, mb);
-                    ma = __viaddmin_u16x2(R.Va[4 * x + 0], c.x, ma);
-                    mb = __viaddmin_u16x2(R.Vb[4 * x + 1], c.y, mb);
-                    ma = __viaddmin_u16x2(R.Va[4 * x + 1], c.y, ma);
-                    mb = __viaddmin_u16x2(R.Vb[4 * x + 2], c.z, mb);
-                    ma = __viaddmin_u16x2(R.Va[4 * x + 2], c.z, ma);
-                    mb = __viaddmin_u16x2(R.Vb[4 * x + 3], c.w, mb);
-                    ma = __viaddmin_u16x2(R.Va[4 * x + 3], c.w, ma);
                 } else {
-                    ma = __viaddmin_u16x2(R.Va[4 * x + 0], c.x, ma);
-                    ma = __viaddmin_u16x2(R.Va[4 * x + 1], c.y, ma);
-                    ma = __viaddmin_u16x2(R.Va[4 * x + 2], c.z, ma);
-                    ma = __viaddmin_u16x2(R.Va[4 * x + 3], c.w, ma);
+                    // fused chunk, register set b before set a for every word of C (order 1 of the table above)
                     mb = __viaddmin_u16x2(R.Vb[4 * x + 0], c.x, mb);
+                    ma = __viaddmin_u16x2(R.Va[4 * x + 0], c.x, ma);
                     mb = __viaddmin_u16x2(R.Vb[4 * x + 1], c.y, mb);
+                    ma = __viaddmin_u16x2(R.Va[4 * x + 1], c.y, ma);
                     mb = __viaddmin_u16x2(R.Vb[4 * x + 2], c.z, mb);
+                    ma = __viaddmin_u16x2(R.Va[4 * x + 2], c.z, ma);
                     mb = __viaddmin_u16x2(R.Vb[4 * x + 3], c.w, mb);
+                    ma = __viaddmin_u16x2(R.Va[4 * x + 3], c.w, ma);
                 }
                 if (r == NHALF / 2 - 1) {
                     // last row: this chunk of V is not needed any more in this step
