@@ -1080,3 +1080,17 @@ def test_three_way_shard_ranges_through_the_tensor_core_screen(B):
     qm, em = B.ising_merge_lists(torch.cat([p[0] for p in parts]), torch.cat([p[1] for p in parts]), S)
     qo, eo = oracle.lowest(J, h, S)
     assert_exact(B.states_to_numpy(qm), em.cpu().numpy(), qo, eo)
+
+
+# ---------- the paper's own largest runs, as whole spaces ("N = 49, 50"; Fig. 6: N = 50, S = 10^3) ----------
+@pytest.mark.parametrize("N,S,seed", [(50, 1000, 5050), (52, 100, 5252)])
+def test_paper_largest_runs_whole_space(B, N, S, seed):
+    """Complete Gaussian instances of 50 spins (S = 1000, the setting of the paper's Fig. 6) and 52 spins, ALL 2^N
+    states through the default path (about 2 s and 8 s on one B200; the paper reports 24 days for N = 50 on its GPU),
+    element by element against the branch-and-bound oracle (tier 3, pinned to the plain oracle in test_oracle_pins.py)."""
+    J, h = I.complete_gaussian(N, seed=seed)
+    q, e = gpu_lowest(B, J, h, S)
+    st = B.last_stats()
+    assert st.configs == 1 << N and st.kernel_variant == 128 and st.passes == 1
+    qo, eo, _ = oracle.lowest_bnb(J, h, S, spare=16)
+    assert_exact(q, e, qo[:S], eo[:S])
