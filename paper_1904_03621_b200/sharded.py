@@ -63,6 +63,8 @@ def ising_lowest_sharded(J, h, S: int, group=None, solver: Optional[Callable] = 
     solver(J, h, S_local, q_begin, q_end) -> (states int64[S_local], energies float64[S_local]) tensors;
     merger(states int64[n], energies float64[n], S) -> (states[S], energies[S]).
     Defaults: the C-ABI calls `binding.ising_lowest_range` / `binding.ising_merge_lists` (CUDA; no CPU fallback).
+    A merge that must not allocate device memory inside the library: `merger=binding.ising_merge_lists_static`
+    (world x S <= 131072 pairs; include/ising.h says which callers need it).
     device: where this rank computes (default: J's device if it is a tensor, else the current CUDA device when the
     default solver is used, else the CPU); a rank with an empty range builds its buffers there.
     always_exchange: run the all-gather and the merge even with a single rank (exercises the collective path on a
